@@ -1,0 +1,140 @@
+/*
+ * frnn.h -- C ABI of the B200-native fixed-radius nearest-neighbour (FRNN) graph builder.
+ *
+ * Operation (what every entry point computes):
+ *   PAPER.md:31 (section 2): "it is necessary to construct a fixed-radius nearest neighbor (FRNN)
+ *     graph in this embedded space. The FRNN graph has only edges connecting neighboring
+ *     spacepoints residing within a constant radius".
+ *   PAPER.md:69 (section 3.4): "all the neighboring points residing within a certain distance from
+ *     each query spacepoint"; solved by a grid ("cell technique") over a low-dimensional projection
+ *     of the embedding, worst case O(n).
+ *   BASELINE.json north_star: directed edge list, at most k_max nearest per query, (src,dst) sorted.
+ *
+ * Result, for each query row i of an event (readings R1..R10 in DESIGN.md section 2):
+ *   S_i = { j != i : d2(i,j) <= r2 },  r2 = fl32(r*r);
+ *   d2(i,j) = fp32 chain  acc = 0; for d = 0..dim-1: t = fl32(x[i][d]-x[j][d]); acc = fma(t,t,acc);
+ *   if |S_i| > k_max keep the k_max smallest under (d2 ascending, then j ascending);
+ *   emit (src=i, dst=j, d2) for the kept j in ascending j; rows i in ascending order.
+ * The result is exact (not approximate): the grid only prunes candidates.
+ *
+ * Conventions
+ *   - Every pointer is a DEVICE pointer owned by the caller unless marked HOST.  The library never
+ *     allocates or frees caller-visible memory.  frnn_build_ex / frnn_build_batched only enqueue
+ *     work on `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and never synchronise.
+ *   - points: row-major n x dim fp32, base 16-byte aligned, finite values (non-finite coordinates
+ *     are a precondition violation; they can never cause an out-of-bounds access).
+ *   - src/dst are int32 row indices (local to the event in the batched call); counts and offsets
+ *     are int64.  Edges of one call are sorted by (src, dst) ascending and free of duplicates.
+ *   - Return value: FRNN_OK or a negative frnn_status for faults the host can detect; in that case
+ *     no output is touched and nothing is enqueued.  Faults only the device can detect are
+ *     reported in *out_status (device int32): FRNN_OK, or FRNN_ERR_CAPACITY when the edge count
+ *     exceeds edge_capacity; then *out_count holds the needed size and only edges at positions
+ *     < edge_capacity are written.
+ *   - Thread safety: calls using distinct workspaces may run concurrently on distinct streams.
+ *     No C++ exception crosses this boundary.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point fails with
+ *     FRNN_ERR_CUDA.
+ */
+#ifndef FRNN_B200_H
+#define FRNN_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    FRNN_OK = 0,
+    FRNN_ERR_INVALID_ARG = -1,  /* null pointer, n < 0, r < 0 or not finite, k_max < 1, bad offsets */
+    FRNN_ERR_UNSUPPORTED = -2,  /* dim != 8, more than 2^31-1 rows */
+    FRNN_ERR_CAPACITY = -3,     /* device-detected: more edges than edge_capacity */
+    FRNN_ERR_WORKSPACE = -4,    /* workspace_bytes < frnn_workspace_bytes(...) */
+    FRNN_ERR_CUDA = -5          /* a CUDA runtime call failed (or no device) */
+} frnn_status;
+
+/* Library/ABI version: major*10000 + minor*100 + patch. */
+int frnn_version(void);
+
+/* Static string for a frnn_status value (never NULL). */
+const char* frnn_status_string(int status);
+
+/*
+ * Bytes of scratch needed for a call over n_total rows in n_events events (n_events = 1 for
+ * frnn_build_ex).  Depends on the grid chosen from (n_total / n_events); 0 on invalid arguments.
+ * The workspace holds S2..S9 of SURVEY.md section 8(a): cell table, cell-ordered point copy,
+ * permutation, per-row counts and the CSR row pointer.  256-byte aligned base required.
+ */
+size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max);
+
+/*
+ * Grid override for sweeps (process-global, affects later calls and frnn_workspace_bytes):
+ * grid_dims = number of leading coordinates that are binned (1..6), grid_bits = log2 of the
+ * toroidal grid extent per binned coordinate (2..8).  0 restores the automatic choice.  The
+ * result never depends on the grid (R8/R9).  Returns FRNN_OK or FRNN_ERR_INVALID_ARG.
+ */
+int frnn_set_grid(int grid_dims, int grid_bits);
+/* The grid a call over (n_total, n_events) would use. */
+void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits);
+
+/*
+ * The north_star 9-argument form.  Current device, legacy default stream, internally cached
+ * workspace, output capacity assumed n*k_max edges (caller guarantees that much room, or at
+ * least as many edges as the result has -- nothing is written beyond n*k_max).  SYNCHRONOUS:
+ * returns after completion.  out_count is a HOST pointer (here and only here).
+ * Not thread safe (shared cached workspace).
+ */
+int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
+               int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t* out_count /* HOST */);
+
+/*
+ * Full single-event form: asynchronous on cuda_stream.
+ *   out_src/out_dst/out_d2 : room for edge_capacity edges each
+ *   out_count              : device int64, number of edges of the result (even on overflow)
+ *   out_status             : device int32, see above
+ *   out_row_ptr            : optional (may be NULL) device int64[n+1], CSR offsets by src row
+ *   workspace              : device scratch of >= frnn_workspace_bytes(n, 1, dim, k_max) bytes
+ * n == 0 and n == 1 are legal (count 0).  r == 0 is legal (edges between exact duplicates).
+ */
+int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
+                  int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                  int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                  void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Batched events (BASELINE.json config 3): n_events independent events concatenated in `points`;
+ * event e owns rows [event_offsets[e], event_offsets[e+1]) (HOST int64[n_events+1], ascending,
+ * event_offsets[0] == 0).  No cross-event edges.  src/dst are LOCAL to the event.  Edges of event
+ * e occupy [out_edge_offsets[e], out_edge_offsets[e+1]) (device int64[n_events+1]); the total is
+ * out_edge_offsets[n_events].  out_row_ptr (optional) has event_offsets[n_events]+1 entries over
+ * the concatenated rows.  workspace >= frnn_workspace_bytes(total rows, n_events, dim, k_max).
+ */
+int frnn_build_batched(const float* points, const int64_t* event_offsets /* HOST */, int n_events,
+                       int dim, float r, int k_max,
+                       int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                       int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * Host-buffer convenience (the end-to-end call bench.py times as "e2e"): points and all outputs
+ * are HOST pointers (pinned memory makes the copies asynchronous); device staging buffers are
+ * cached inside the library.  Copies the points in, runs frnn_build_ex, copies count + edges
+ * out, synchronises.  Returns FRNN_ERR_CAPACITY if the result has more than edge_capacity edges
+ * (*out_count = needed size, nothing else copied).  Not thread safe.
+ */
+int frnn_build_host(const float* points /* HOST */, int64_t n, int dim, float r, int k_max,
+                    int32_t* out_src /* HOST */, int32_t* out_dst /* HOST */, float* out_d2 /* HOST */,
+                    int64_t edge_capacity, int64_t* out_count /* HOST */);
+
+/* Number of kernel launches (memset nodes included) the last frnn_build_ex/_batched call enqueued
+ * on this thread; what bench.py reports as gpu_launches. */
+int frnn_last_launch_count(void);
+
+/* Release the cached workspace / staging buffers of frnn_build and frnn_build_host. */
+void frnn_release_cached(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FRNN_B200_H */

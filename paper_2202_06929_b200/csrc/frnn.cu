@@ -1,0 +1,363 @@
+// frnn.cu -- host side of the C ABI declared in include/frnn.h (argument checks, workspace layout,
+// launch sequence).  No CPU fallback: every compute entry point needs a CUDA device.
+#include "frnn_kernels.cuh"
+
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/frnn.h"
+
+namespace {
+
+using namespace frnn;
+
+constexpr float kCellSlack = 1.0078125f;   // 1 + 2^-7, see cell_coord()
+constexpr size_t kAlign = 256;
+
+int g_force_dims = 0, g_force_bits = 0;
+thread_local int t_launches = 0;
+
+struct GridChoice { int dims, bits; };
+
+// Grid heuristic: cells per event = 2^(dims*bits).  Finer grids cut candidate rows per query
+// (3^dims cells of side ~r are visited) but cost table size and run bookkeeping; the switch points
+// come from the sweep recorded in DESIGN.md section 7.
+GridChoice choose_grid(int64_t n_total, int n_events) {
+    const int64_t per_event = n_events > 0 ? (n_total + n_events - 1) / n_events : n_total;
+    GridChoice g;
+    g.bits = g_force_bits ? g_force_bits : 5;
+    if (g_force_dims) g.dims = g_force_dims;
+    else if (per_event < 16384) g.dims = 3;
+    else if (per_event < 400000) g.dims = 4;
+    else g.dims = 5;
+    int ev_bits = 0;
+    while ((1ll << ev_bits) < n_events) ++ev_bits;
+    while (g.dims * g.bits + ev_bits > 31 && g.dims > 1) --g.dims;     // linear cell id is 32-bit
+    while (g.dims * g.bits + ev_bits > 31 && g.bits > 2) --g.bits;
+    return g;
+}
+
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    int64_t n_cells, tiles_a, tiles_b;
+    size_t off_cells, off_tiles_a, off_tiles_b, off_counters, zero_bytes;
+    size_t off_pcell, off_prank, off_spts, off_sidx, off_cnt, off_rowptr, off_evoff, off_segs, off_count;
+    size_t total;
+};
+
+Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
+    Layout L;
+    L.n_cells = static_cast<int64_t>(n_events) << (g.dims * g.bits);
+    L.tiles_a = (L.n_cells + kScanTile - 1) / kScanTile;
+    L.tiles_b = (n_total + kScanTile - 1) / kScanTile;
+    size_t o = 0;
+    L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_cells + 1) * 4);
+    L.off_tiles_a = o;  o = align_up(o + static_cast<size_t>(L.tiles_a) * 8);
+    L.off_tiles_b = o;  o = align_up(o + static_cast<size_t>(L.tiles_b > 0 ? L.tiles_b : 1) * 8);
+    L.off_counters = o; o = align_up(o + 64);
+    L.zero_bytes = o;
+    const size_t n = static_cast<size_t>(n_total > 0 ? n_total : 1);
+    const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
+    L.off_pcell = o;  o = align_up(o + n * 4);
+    L.off_prank = o;  o = align_up(o + n * 4);
+    L.off_spts = o;   o = align_up(o + n * 32);
+    L.off_sidx = o;   o = align_up(o + n * 4);
+    L.off_cnt = o;    o = align_up(o + n * 4);
+    L.off_rowptr = o; o = align_up(o + (n + 1) * 8);
+    L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
+    L.off_segs = o;   o = align_up(o + static_cast<size_t>(max_segs > 0 ? max_segs : 1) * sizeof(Segment));
+    L.off_count = o;  o = align_up(o + 64);
+    L.total = o;
+    return L;
+}
+
+int g_num_sms = 0;
+int num_sms() {
+    if (!g_num_sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    return g_num_sms;
+}
+
+template <int G, int PASS>
+cudaError_t launch_search(const SearchArgs& a, int64_t max_segs, cudaStream_t st) {
+    static int blocks_per_sm = 0;
+    if (!blocks_per_sm) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, search_kernel<G, PASS>, kSearchWarps * 32, 0) != cudaSuccess ||
+            blocks_per_sm < 1)
+            blocks_per_sm = 1;
+    }
+    int64_t blocks = (max_segs + kSearchWarps - 1) / kSearchWarps;
+    const int64_t resident = static_cast<int64_t>(num_sms()) * blocks_per_sm;
+    if (blocks > resident) blocks = resident;
+    if (blocks < 1) blocks = 1;
+    search_kernel<G, PASS><<<static_cast<unsigned>(blocks), kSearchWarps * 32, 0, st>>>(a);
+    ++t_launches;
+    return cudaGetLastError();
+}
+
+template <int G>
+cudaError_t launch_bin(const float* pts, int64_t n, const int64_t* ev_off, int n_events, float inv_cell, int bits,
+                       uint32_t* cells, uint32_t* pcell, uint32_t* prank, cudaStream_t st) {
+    bin_kernel<G><<<static_cast<unsigned>((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(pts), n, ev_off, n_events,
+                                                                        inv_cell, bits, cells, pcell, prank);
+    ++t_launches;
+    return cudaGetLastError();
+}
+
+#define FRNN_DISPATCH_G(G_, EXPR)          \
+    switch (G_) {                          \
+        case 1: { constexpr int GG = 1; EXPR; } break; \
+        case 2: { constexpr int GG = 2; EXPR; } break; \
+        case 3: { constexpr int GG = 3; EXPR; } break; \
+        case 4: { constexpr int GG = 4; EXPR; } break; \
+        case 5: { constexpr int GG = 5; EXPR; } break; \
+        default: { constexpr int GG = 6; EXPR; } break; \
+    }
+
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return FRNN_ERR_CUDA; } while (0)
+
+int check_common(const float* points, int64_t n, int dim, float r, int k_max, const void* out_src, const void* out_dst,
+                 const void* out_d2, int64_t capacity) {
+    if (n < 0 || k_max < 1 || capacity < 0) return FRNN_ERR_INVALID_ARG;
+    if (!(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
+    if (n > 0 && !points) return FRNN_ERR_INVALID_ARG;
+    if (capacity > 0 && (!out_src || !out_dst || !out_d2)) return FRNN_ERR_INVALID_ARG;
+    if (dim != kDim) return FRNN_ERR_UNSUPPORTED;
+    if (n > 0x7fffffffll) return FRNN_ERR_UNSUPPORTED;
+    return FRNN_OK;
+}
+
+// The whole path, enqueued on `st`.  ev_off_host has n_events+1 entries.
+int enqueue(const float* points, const int64_t* ev_off_host, int n_events, float r, int k_max,
+            int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t capacity,
+            int64_t* out_count, int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
+            void* workspace, size_t workspace_bytes, cudaStream_t st) {
+    t_launches = 0;
+    const int64_t n_total = ev_off_host[n_events];
+    if (n_total == 0) {                       // nothing to search: zero the outputs and leave
+        if (out_count) { CK(cudaMemsetAsync(out_count, 0, 8, st)); ++t_launches; }
+        if (out_edge_offsets) { CK(cudaMemsetAsync(out_edge_offsets, 0, 8 * static_cast<size_t>(n_events + 1), st)); ++t_launches; }
+        if (out_row_ptr) { CK(cudaMemsetAsync(out_row_ptr, 0, 8, st)); ++t_launches; }
+        CK(cudaMemsetAsync(out_status, 0, 4, st)); ++t_launches;
+        return FRNN_OK;
+    }
+    const GridChoice g = choose_grid(n_total, n_events);
+    const Layout L = make_layout(n_total, n_events, g);
+    if (!workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
+    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return FRNN_ERR_INVALID_ARG;
+    char* ws = static_cast<char*>(workspace);
+    uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
+    uint64_t* tiles_a = reinterpret_cast<uint64_t*>(ws + L.off_tiles_a);
+    uint64_t* tiles_b = reinterpret_cast<uint64_t*>(ws + L.off_tiles_b);
+    uint32_t* counters = reinterpret_cast<uint32_t*>(ws + L.off_counters);   // [0] ticket A, [1] ticket B, [2] n_segs
+    uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
+    uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
+    float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
+    int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
+    uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
+    int64_t* row_ptr = out_row_ptr ? out_row_ptr : reinterpret_cast<int64_t*>(ws + L.off_rowptr);
+    int64_t* ev_off = reinterpret_cast<int64_t*>(ws + L.off_evoff);
+    Segment* segs = reinterpret_cast<Segment*>(ws + L.off_segs);
+
+    const float r2 = r * r;                                   // R2: fl32(r*r), once, on the host
+    const float cell_side = fmaxf(r * kCellSlack, 1e-30f);
+    const float inv_cell = 1.0f / cell_side;
+
+    CK(cudaMemsetAsync(ws, 0, L.zero_bytes, st)); ++t_launches;
+    // Event offsets reach the device as kernel arguments (no pageable-memory copy, which would
+    // synchronise the host with the stream); a single event needs none (base 0).
+    if (n_events > 1) {
+        for (int first = 0; first <= n_events; first += OffsetChunk::kN) {
+            OffsetChunk c;
+            c.first = first;
+            c.count = (n_events + 1 - first) < OffsetChunk::kN ? (n_events + 1 - first) : OffsetChunk::kN;
+            for (int k = 0; k < c.count; ++k) c.v[k] = ev_off_host[first + k];
+            set_offsets_kernel<<<1, OffsetChunk::kN, 0, st>>>(c, ev_off);
+            ++t_launches; CK(cudaGetLastError());
+        }
+    } else {
+        ev_off = nullptr;
+    }
+
+    FRNN_DISPATCH_G(g.dims, CK(launch_bin<GG>(points, n_total, ev_off, n_events, inv_cell, g.bits, cells, pcell, prank, st)));
+
+    scan_kernel<CellScan><<<static_cast<unsigned>(L.tiles_a), kScanThreads, 0, st>>>(CellScan{cells, segs, counters + 2}, L.n_cells,
+                                                                                   tiles_a, counters + 0);
+    ++t_launches; CK(cudaGetLastError());
+
+    scatter_kernel<<<static_cast<unsigned>((n_total + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(points), n_total, cells,
+                                                                               pcell, prank, spts, sidx);
+    ++t_launches; CK(cudaGetLastError());
+
+    SearchArgs a;
+    a.spts = spts; a.sidx = sidx; a.cell_start = cells; a.segs = segs; a.n_segs = counters + 2; a.ev_off = ev_off;
+    a.cnt = cnt; a.row_ptr = row_ptr; a.out_src = out_src; a.out_dst = out_dst; a.out_d2 = out_d2;
+    a.capacity = capacity; a.r2 = r2; a.bits = g.bits; a.k_max = static_cast<uint32_t>(k_max);
+    const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
+
+    FRNN_DISPATCH_G(g.dims, CK((launch_search<GG, 0>(a, max_segs, st))));
+
+    scan_kernel<DegreeScan><<<static_cast<unsigned>(L.tiles_b), kScanThreads, 0, st>>>(DegreeScan{cnt, row_ptr, static_cast<uint32_t>(k_max)},
+                                                                                     n_total, tiles_b, counters + 1);
+    ++t_launches; CK(cudaGetLastError());
+
+    FRNN_DISPATCH_G(g.dims, CK((launch_search<GG, 1>(a, max_segs, st))));
+
+    sort_rows_kernel<<<static_cast<unsigned>((n_total + 255) / 256), 256, 0, st>>>(row_ptr, n_total, capacity, out_dst, out_d2, ev_off,
+                                                                                 n_events, out_count, out_edge_offsets, out_status);
+    ++t_launches; CK(cudaGetLastError());
+    return FRNN_OK;
+}
+
+// cached device buffers for the synchronous convenience entry points
+struct Cache {
+    void* ws = nullptr; size_t ws_bytes = 0;
+    void* misc = nullptr;                       // count (8) + status (4)
+    void* pts = nullptr; size_t pts_bytes = 0;
+    void* edges = nullptr; size_t edge_cap = 0; // src | dst | d2, edge_cap each
+} g_cache;
+
+int ensure(void** p, size_t* have, size_t need) {
+    if (*have >= need && *p) return FRNN_OK;
+    if (*p) cudaFree(*p);
+    *p = nullptr; *have = 0;
+    if (cudaMalloc(p, need) != cudaSuccess) return FRNN_ERR_CUDA;
+    *have = need;
+    return FRNN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int frnn_version(void) { return 100; }   // 0.1.0
+
+const char* frnn_status_string(int status) {
+    switch (status) {
+        case FRNN_OK: return "ok";
+        case FRNN_ERR_INVALID_ARG: return "invalid argument";
+        case FRNN_ERR_UNSUPPORTED: return "unsupported (dim != 8 or too many rows)";
+        case FRNN_ERR_CAPACITY: return "edge capacity exceeded";
+        case FRNN_ERR_WORKSPACE: return "workspace too small";
+        case FRNN_ERR_CUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max) {
+    if (n_total < 0 || n_events < 1 || dim != kDim || k_max < 1 || n_total > 0x7fffffffll) return 0;
+    return make_layout(n_total, n_events, choose_grid(n_total, n_events)).total;
+}
+
+int frnn_set_grid(int grid_dims, int grid_bits) {
+    if (grid_dims < 0 || grid_dims > 6 || (grid_bits != 0 && (grid_bits < 2 || grid_bits > 8))) return FRNN_ERR_INVALID_ARG;
+    g_force_dims = grid_dims;
+    g_force_bits = grid_bits;
+    return FRNN_OK;
+}
+
+void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits) {
+    const GridChoice g = choose_grid(n_total, n_events < 1 ? 1 : n_events);
+    if (grid_dims) *grid_dims = g.dims;
+    if (grid_bits) *grid_bits = g.bits;
+}
+
+int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
+                  int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                  int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                  void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    if (rc != FRNN_OK) return rc;
+    if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
+    const int64_t ev_off[2] = {0, n};
+    return enqueue(points, ev_off, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status,
+                   out_row_ptr, workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int frnn_build_batched(const float* points, const int64_t* event_offsets, int n_events, int dim, float r, int k_max,
+                       int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                       int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (n_events < 1 || !event_offsets || event_offsets[0] != 0) return FRNN_ERR_INVALID_ARG;
+    for (int e = 0; e < n_events; ++e)
+        if (event_offsets[e + 1] < event_offsets[e]) return FRNN_ERR_INVALID_ARG;
+    int rc = check_common(points, event_offsets[n_events], dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    if (rc != FRNN_OK) return rc;
+    if (!out_edge_offsets || !out_status) return FRNN_ERR_INVALID_ARG;
+    return enqueue(points, event_offsets, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets,
+                   out_status, out_row_ptr, workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
+               int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t* out_count) {
+    if (!out_count) return FRNN_ERR_INVALID_ARG;
+    const int64_t cap = n > 0 ? n * static_cast<int64_t>(k_max > 0 ? k_max : 0) : 0;
+    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, cap);
+    if (rc != FRNN_OK) return rc;
+    const size_t need = frnn_workspace_bytes(n, 1, dim, k_max);
+    size_t misc_have = g_cache.misc ? 64 : 0;
+    if ((rc = ensure(&g_cache.ws, &g_cache.ws_bytes, need)) != FRNN_OK) return rc;
+    if ((rc = ensure(&g_cache.misc, &misc_have, 64)) != FRNN_OK) return rc;
+    int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
+    int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
+    rc = frnn_build_ex(points, n, dim, r, k_max, out_src, out_dst, out_d2, cap, d_count, d_status, nullptr, g_cache.ws,
+                       g_cache.ws_bytes, nullptr);
+    if (rc != FRNN_OK) return rc;
+    int32_t h_status = 0;
+    CK(cudaMemcpy(out_count, d_count, 8, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(&h_status, d_status, 4, cudaMemcpyDeviceToHost));
+    return h_status;
+}
+
+int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
+                    int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity, int64_t* out_count) {
+    if (!out_count) return FRNN_ERR_INVALID_ARG;
+    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    if (rc != FRNN_OK) return rc;
+    const size_t need = frnn_workspace_bytes(n, 1, dim, k_max);
+    size_t misc_have = g_cache.misc ? 64 : 0;
+    size_t edge_bytes = g_cache.edge_cap * 12;
+    if ((rc = ensure(&g_cache.ws, &g_cache.ws_bytes, need)) != FRNN_OK) return rc;
+    if ((rc = ensure(&g_cache.misc, &misc_have, 64)) != FRNN_OK) return rc;
+    if ((rc = ensure(&g_cache.pts, &g_cache.pts_bytes, static_cast<size_t>(n > 0 ? n : 1) * 32)) != FRNN_OK) return rc;
+    if (g_cache.edge_cap < static_cast<size_t>(edge_capacity) || !g_cache.edges) {
+        if ((rc = ensure(&g_cache.edges, &edge_bytes, static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1) * 12)) != FRNN_OK) return rc;
+        g_cache.edge_cap = static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1);
+    }
+    int32_t* d_src = static_cast<int32_t*>(g_cache.edges);
+    int32_t* d_dst = d_src + g_cache.edge_cap;
+    float* d_d2 = reinterpret_cast<float*>(d_dst + g_cache.edge_cap);
+    int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
+    int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
+    if (n > 0) CK(cudaMemcpyAsync(g_cache.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, nullptr));
+    rc = frnn_build_ex(static_cast<const float*>(g_cache.pts), n, dim, r, k_max, d_src, d_dst, d_d2, edge_capacity, d_count, d_status,
+                       nullptr, g_cache.ws, g_cache.ws_bytes, nullptr);
+    if (rc != FRNN_OK) return rc;
+    CK(cudaMemcpy(out_count, d_count, 8, cudaMemcpyDeviceToHost));
+    if (*out_count > edge_capacity) return FRNN_ERR_CAPACITY;
+    const size_t e = static_cast<size_t>(*out_count);
+    if (e) {
+        CK(cudaMemcpyAsync(out_src, d_src, e * 4, cudaMemcpyDeviceToHost, nullptr));
+        CK(cudaMemcpyAsync(out_dst, d_dst, e * 4, cudaMemcpyDeviceToHost, nullptr));
+        CK(cudaMemcpyAsync(out_d2, d_d2, e * 4, cudaMemcpyDeviceToHost, nullptr));
+        CK(cudaStreamSynchronize(nullptr));
+    }
+    return FRNN_OK;
+}
+
+int frnn_last_launch_count(void) { return t_launches; }
+
+void frnn_release_cached(void) {
+    if (g_cache.ws) cudaFree(g_cache.ws);
+    if (g_cache.misc) cudaFree(g_cache.misc);
+    if (g_cache.pts) cudaFree(g_cache.pts);
+    if (g_cache.edges) cudaFree(g_cache.edges);
+    g_cache = Cache{};
+}
+
+}  // extern "C"

@@ -1,0 +1,232 @@
+"""Thin ctypes binding of include/frnn.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of ``libfrnn_b200.so``; PyTorch is used for device
+memory and streams.  There is no CPU fallback: a missing library or a missing CUDA device raises.
+Function names mirror the C ABI.  Operation: PAPER.md:31 (section 2), PAPER.md:69 (section 3.4).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+from . import build as _build
+
+FRNN_OK = 0
+FRNN_ERR_INVALID_ARG = -1
+FRNN_ERR_UNSUPPORTED = -2
+FRNN_ERR_CAPACITY = -3
+FRNN_ERR_WORKSPACE = -4
+FRNN_ERR_CUDA = -5
+
+_c = ctypes
+_SIGNATURES = {
+    "frnn_version": (_c.c_int, []),
+    "frnn_status_string": (_c.c_char_p, [_c.c_int]),
+    "frnn_workspace_bytes": (_c.c_size_t, [_c.c_int64, _c.c_int, _c.c_int, _c.c_int]),
+    "frnn_set_grid": (_c.c_int, [_c.c_int, _c.c_int]),
+    "frnn_get_grid": (None, [_c.c_int64, _c.c_int, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int)]),
+    "frnn_build": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
+                              _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.POINTER(_c.c_int64)]),
+    "frnn_build_ex": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
+                                 _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
+                                 _c.c_void_p, _c.c_void_p, _c.c_void_p,
+                                 _c.c_void_p, _c.c_size_t, _c.c_void_p]),
+    "frnn_build_batched": (_c.c_int, [_c.c_void_p, _c.POINTER(_c.c_int64), _c.c_int, _c.c_int, _c.c_float, _c.c_int,
+                                      _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
+                                      _c.c_void_p, _c.c_void_p, _c.c_void_p,
+                                      _c.c_void_p, _c.c_size_t, _c.c_void_p]),
+    "frnn_build_host": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
+                                   _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64, _c.POINTER(_c.c_int64)]),
+    "frnn_last_launch_count": (_c.c_int, []),
+    "frnn_release_cached": (None, []),
+}
+EXPORTED_SYMBOLS = tuple(_SIGNATURES)
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building first if the sources are newer) the C-ABI shared library.  Raises if absent."""
+    global _lib
+    if _lib is None:
+        path = _build.build() if os.path.exists(_build.SOURCES[0]) else _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing: the CUDA extension is required (no CPU fallback)")
+        handle = ctypes.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(handle, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = handle
+    return _lib
+
+
+class FrnnError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {frnn_status_string(status)} ({status})")
+
+
+def _check(status: int, where: str):
+    if status != FRNN_OK:
+        raise FrnnError(status, where)
+
+
+def frnn_version() -> int:
+    return lib().frnn_version()
+
+
+def frnn_status_string(status: int) -> str:
+    return lib().frnn_status_string(int(status)).decode()
+
+
+def frnn_workspace_bytes(n_total: int, n_events: int = 1, dim: int = 8, k_max: int = 1) -> int:
+    return int(lib().frnn_workspace_bytes(int(n_total), int(n_events), int(dim), int(k_max)))
+
+
+def frnn_set_grid(grid_dims: int = 0, grid_bits: int = 0) -> None:
+    _check(lib().frnn_set_grid(int(grid_dims), int(grid_bits)), "frnn_set_grid")
+
+
+def frnn_get_grid(n_total: int, n_events: int = 1) -> tuple[int, int]:
+    d, b = _c.c_int(0), _c.c_int(0)
+    lib().frnn_get_grid(int(n_total), int(n_events), _c.byref(d), _c.byref(b))
+    return d.value, b.value
+
+
+def frnn_last_launch_count() -> int:
+    return lib().frnn_last_launch_count()
+
+
+def frnn_release_cached() -> None:
+    lib().frnn_release_cached()
+
+
+def _require_cuda(points: torch.Tensor):
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2202_06929_b200 needs a CUDA device (no CPU fallback)")
+    if not (points.is_cuda and points.dtype == torch.float32 and points.is_contiguous() and points.dim() == 2):
+        raise ValueError("points must be a contiguous CUDA float32 tensor of shape (n, dim)")
+
+
+def _ptr(t):
+    return None if t is None else _c.c_void_p(t.data_ptr())
+
+
+@dataclass
+class EdgeList:
+    """Device-resident result.  ``src/dst/d2`` have ``edge_capacity`` entries; the first ``count``
+    (device scalar; ``n_edges()`` synchronises) are valid and (src,dst)-sorted."""
+    src: torch.Tensor
+    dst: torch.Tensor
+    d2: torch.Tensor
+    count: torch.Tensor             # int64[1] (single event) or int64[B+1] edge offsets (batched)
+    status: torch.Tensor            # int32[1]
+    row_ptr: torch.Tensor | None
+
+    def n_edges(self) -> int:
+        return int(self.count[-1].item())
+
+    def check(self):
+        st = int(self.status.item())
+        if st != FRNN_OK:
+            raise FrnnError(st, "device status")
+        return self
+
+    def trimmed(self):
+        e = self.n_edges()
+        return self.src[:e], self.dst[:e], self.d2[:e]
+
+
+class Workspace:
+    """Reusable device scratch + output buffers for repeated calls of one shape."""
+
+    def __init__(self, n_total: int, n_events: int, k_max: int, edge_capacity: int, device=None, want_row_ptr: bool = False):
+        device = device or torch.device("cuda", torch.cuda.current_device())
+        self.bytes = frnn_workspace_bytes(n_total, n_events, 8, k_max)
+        self.buf = torch.empty(max(self.bytes, 256), dtype=torch.uint8, device=device)
+        self.edge_capacity = int(edge_capacity)
+        cap = max(self.edge_capacity, 1)
+        self.src = torch.empty(cap, dtype=torch.int32, device=device)
+        self.dst = torch.empty(cap, dtype=torch.int32, device=device)
+        self.d2 = torch.empty(cap, dtype=torch.float32, device=device)
+        self.count = torch.zeros(n_events + 1 if n_events > 1 else 1, dtype=torch.int64, device=device)
+        self.status = torch.zeros(1, dtype=torch.int32, device=device)
+        self.row_ptr = torch.empty(n_total + 1, dtype=torch.int64, device=device) if want_row_ptr else None
+
+
+def frnn_build_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int | None = None,
+                  ws: Workspace | None = None, stream: torch.cuda.Stream | None = None,
+                  want_row_ptr: bool = False) -> EdgeList:
+    """Asynchronous single-event build on ``stream`` (default: torch's current stream)."""
+    _require_cuda(points)
+    n, dim = points.shape
+    if edge_capacity is None:
+        edge_capacity = ws.edge_capacity if ws is not None else n * k_max
+    if ws is None:
+        ws = Workspace(n, 1, k_max, edge_capacity, points.device, want_row_ptr)
+    stream = stream or torch.cuda.current_stream(points.device)
+    st = lib().frnn_build_ex(_ptr(points), n, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst), _ptr(ws.d2),
+                             int(edge_capacity), _ptr(ws.count), _ptr(ws.status), _ptr(ws.row_ptr),
+                             _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    _check(st, "frnn_build_ex")
+    return EdgeList(ws.src, ws.dst, ws.d2, ws.count, ws.status, ws.row_ptr)
+
+
+def frnn_build_batched(points: torch.Tensor, event_offsets, r: float, k_max: int, edge_capacity: int | None = None,
+                       ws: Workspace | None = None, stream: torch.cuda.Stream | None = None,
+                       want_row_ptr: bool = False) -> EdgeList:
+    """Asynchronous batched build: ``event_offsets`` is a host sequence of B+1 ascending row offsets."""
+    _require_cuda(points)
+    n, dim = points.shape
+    offs = [int(v) for v in event_offsets]
+    n_events = len(offs) - 1
+    if edge_capacity is None:
+        edge_capacity = ws.edge_capacity if ws is not None else n * k_max
+    if ws is None:
+        ws = Workspace(n, n_events, k_max, edge_capacity, points.device, want_row_ptr)
+    count = ws.count if ws.count.numel() == n_events + 1 else torch.zeros(n_events + 1, dtype=torch.int64, device=points.device)
+    stream = stream or torch.cuda.current_stream(points.device)
+    c_offs = (_c.c_int64 * (n_events + 1))(*offs)
+    st = lib().frnn_build_batched(_ptr(points), c_offs, n_events, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst),
+                                  _ptr(ws.d2), int(edge_capacity), _ptr(count), _ptr(ws.status), _ptr(ws.row_ptr),
+                                  _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    _check(st, "frnn_build_batched")
+    return EdgeList(ws.src, ws.dst, ws.d2, count, ws.status, ws.row_ptr)
+
+
+def frnn_build(points: torch.Tensor, r: float, k_max: int):
+    """The synchronous 9-argument form: returns trimmed (src, dst, d2) device tensors."""
+    _require_cuda(points)
+    n, dim = points.shape
+    cap = max(n * k_max, 1)
+    src = torch.empty(cap, dtype=torch.int32, device=points.device)
+    dst = torch.empty(cap, dtype=torch.int32, device=points.device)
+    d2 = torch.empty(cap, dtype=torch.float32, device=points.device)
+    count = _c.c_int64(0)
+    torch.cuda.current_stream(points.device).synchronize()      # the C call uses the legacy default stream
+    st = lib().frnn_build(_ptr(points), n, dim, float(r), int(k_max), _ptr(src), _ptr(dst), _ptr(d2), _c.byref(count))
+    _check(st, "frnn_build")
+    e = count.value
+    return src[:e], dst[:e], d2[:e]
+
+
+def frnn_build_host(points_host: torch.Tensor, r: float, k_max: int, out_src: torch.Tensor, out_dst: torch.Tensor,
+                    out_d2: torch.Tensor) -> int:
+    """End-to-end call on HOST tensors (pinned recommended): H2D, build, D2H.  Returns the edge count."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2202_06929_b200 needs a CUDA device (no CPU fallback)")
+    assert not points_host.is_cuda and points_host.dtype == torch.float32 and points_host.is_contiguous()
+    n, dim = points_host.shape
+    cap = min(out_src.numel(), out_dst.numel(), out_d2.numel())
+    count = _c.c_int64(0)
+    st = lib().frnn_build_host(_ptr(points_host), n, dim, float(r), int(k_max), _ptr(out_src), _ptr(out_dst), _ptr(out_d2),
+                               cap, _c.byref(count))
+    _check(st, "frnn_build_host")
+    return count.value
