@@ -131,6 +131,18 @@ int frnn_build_host(const float* points /* HOST */, int64_t n, int dim, float r,
  * on this thread; what bench.py reports as gpu_launches. */
 int frnn_last_launch_count(void);
 
+/*
+ * Per-phase device timing for bench.py's roofline line.  frnn_set_profiling(1) makes every later
+ * frnn_build_ex/_batched call record one CUDA event after each phase of the path (on the call's
+ * stream); frnn_get_profile waits for the LAST profiled call and writes the duration in ms of
+ * each phase (memset, bin, scan_cells, scatter, search_count, scan_degrees, search_write,
+ * sort_rows) into phase_ms[0..max_phases), returning the number of phases written or a negative
+ * status.  Process-global, not thread safe; leave it off when timing whole calls.
+ */
+int frnn_set_profiling(int enabled);
+int frnn_get_profile(float* phase_ms /* HOST */, int max_phases);
+const char* frnn_phase_name(int phase);
+
 /* Release the cached workspace / staging buffers of frnn_build and frnn_build_host. */
 void frnn_release_cached(void);
 

@@ -18,6 +18,17 @@ constexpr size_t kAlign = 256;
 int g_force_dims = 0, g_force_bits = 0;
 thread_local int t_launches = 0;
 
+// Optional per-phase CUDA-event timing (frnn_set_profiling): one event after every phase.
+constexpr int kPhases = 8;
+const char* const kPhaseNames[kPhases] = {"memset", "bin", "scan_cells", "scatter", "search_count", "scan_degrees",
+                                          "search_write", "sort_rows"};
+bool g_profiling = false;
+cudaEvent_t g_ev[kPhases + 1] = {};
+bool g_ev_valid = false;
+void mark(int phase_done, cudaStream_t st) {        // phase_done = -1: start of the call
+    if (g_profiling && g_ev_valid) cudaEventRecord(g_ev[phase_done + 1], st);
+}
+
 struct GridChoice { int dims, bits; };
 
 // Grid heuristic: cells per event = 2^(dims*bits).  Finer grids cut candidate rows per query
@@ -168,6 +179,7 @@ int enqueue(const float* points, const int64_t* ev_off_host, int n_events, float
     const float cell_side = fmaxf(r * kCellSlack, 1e-30f);
     const float inv_cell = 1.0f / cell_side;
 
+    mark(-1, st);
     CK(cudaMemsetAsync(ws, 0, L.zero_bytes, st)); ++t_launches;
     // Event offsets reach the device as kernel arguments (no pageable-memory copy, which would
     // synchronise the host with the stream); a single event needs none (base 0).
@@ -184,15 +196,19 @@ int enqueue(const float* points, const int64_t* ev_off_host, int n_events, float
         ev_off = nullptr;
     }
 
+    mark(0, st);
     FRNN_DISPATCH_G(g.dims, CK(launch_bin<GG>(points, n_total, ev_off, n_events, inv_cell, g.bits, cells, pcell, prank, st)));
+    mark(1, st);
 
     scan_kernel<CellScan><<<static_cast<unsigned>(L.tiles_a), kScanThreads, 0, st>>>(CellScan{cells, segs, counters + 2}, L.n_cells,
                                                                                    tiles_a, counters + 0);
     ++t_launches; CK(cudaGetLastError());
+    mark(2, st);
 
     scatter_kernel<<<static_cast<unsigned>((n_total + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(points), n_total, cells,
                                                                                pcell, prank, spts, sidx);
     ++t_launches; CK(cudaGetLastError());
+    mark(3, st);
 
     SearchArgs a;
     a.spts = spts; a.sidx = sidx; a.cell_start = cells; a.segs = segs; a.n_segs = counters + 2; a.ev_off = ev_off;
@@ -201,16 +217,20 @@ int enqueue(const float* points, const int64_t* ev_off_host, int n_events, float
     const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
 
     FRNN_DISPATCH_G(g.dims, CK((launch_search<GG, 0>(a, max_segs, st))));
+    mark(4, st);
 
     scan_kernel<DegreeScan><<<static_cast<unsigned>(L.tiles_b), kScanThreads, 0, st>>>(DegreeScan{cnt, row_ptr, static_cast<uint32_t>(k_max)},
                                                                                      n_total, tiles_b, counters + 1);
     ++t_launches; CK(cudaGetLastError());
+    mark(5, st);
 
     FRNN_DISPATCH_G(g.dims, CK((launch_search<GG, 1>(a, max_segs, st))));
+    mark(6, st);
 
     sort_rows_kernel<<<static_cast<unsigned>((n_total + 255) / 256), 256, 0, st>>>(row_ptr, n_total, capacity, out_dst, out_d2, ev_off,
                                                                                  n_events, out_count, out_edge_offsets, out_status);
     ++t_launches; CK(cudaGetLastError());
+    mark(7, st);
     return FRNN_OK;
 }
 
@@ -351,6 +371,27 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
 }
 
 int frnn_last_launch_count(void) { return t_launches; }
+
+int frnn_set_profiling(int enabled) {
+    if (enabled && !g_ev_valid) {
+        for (int i = 0; i <= kPhases; ++i)
+            if (cudaEventCreate(&g_ev[i]) != cudaSuccess) return FRNN_ERR_CUDA;
+        g_ev_valid = true;
+    }
+    g_profiling = enabled != 0;
+    return FRNN_OK;
+}
+
+int frnn_get_profile(float* phase_ms, int max_phases) {
+    if (!g_ev_valid || !phase_ms) return FRNN_ERR_INVALID_ARG;
+    if (cudaEventSynchronize(g_ev[kPhases]) != cudaSuccess) return FRNN_ERR_CUDA;
+    const int n = max_phases < kPhases ? max_phases : kPhases;
+    for (int i = 0; i < n; ++i)
+        if (cudaEventElapsedTime(&phase_ms[i], g_ev[i], g_ev[i + 1]) != cudaSuccess) return FRNN_ERR_CUDA;
+    return n;
+}
+
+const char* frnn_phase_name(int phase) { return (phase >= 0 && phase < kPhases) ? kPhaseNames[phase] : ""; }
 
 void frnn_release_cached(void) {
     if (g_cache.ws) cudaFree(g_cache.ws);

@@ -41,6 +41,9 @@ _SIGNATURES = {
     "frnn_build_host": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
                                    _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64, _c.POINTER(_c.c_int64)]),
     "frnn_last_launch_count": (_c.c_int, []),
+    "frnn_set_profiling": (_c.c_int, [_c.c_int]),
+    "frnn_get_profile": (_c.c_int, [_c.POINTER(_c.c_float), _c.c_int]),
+    "frnn_phase_name": (_c.c_char_p, [_c.c_int]),
     "frnn_release_cached": (None, []),
 }
 EXPORTED_SYMBOLS = tuple(_SIGNATURES)
@@ -102,6 +105,19 @@ def frnn_get_grid(n_total: int, n_events: int = 1) -> tuple[int, int]:
 
 def frnn_last_launch_count() -> int:
     return lib().frnn_last_launch_count()
+
+
+def frnn_set_profiling(enabled: bool) -> None:
+    _check(lib().frnn_set_profiling(int(bool(enabled))), "frnn_set_profiling")
+
+
+def frnn_get_profile() -> dict[str, float]:
+    """Per-phase milliseconds of the last profiled call (synchronises on it)."""
+    buf = (_c.c_float * 16)()
+    n = lib().frnn_get_profile(buf, 16)
+    if n < 0:
+        raise FrnnError(n, "frnn_get_profile")
+    return {lib().frnn_phase_name(i).decode(): float(buf[i]) for i in range(n)}
 
 
 def frnn_release_cached() -> None:
