@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- FRNN graph building at tracking scale (BASELINE.json: 120k hits, D=8, r=0.1, K=256).
 
-One "step" = one pass of the whole hot path (S2..S10: bin, scan, scatter, count, scan, write, sort)
+One "step" = one pass of the whole hot path (S2..S10: bin, cell scan, scatter, search, degree scan + emit)
 over ONE seeded synthetic event of config 2 through the C ABI (frnn_build_ex) on a non-default
 stream.  Steps rotate over a pool of distinct events and distinct output buffers whose total size
 exceeds the 126 MB L2, so every step reads its input cold from HBM.
@@ -281,8 +281,9 @@ def main() -> None:
     cand = float(np.mean([candidate_rows(host_events[i], r, dims, bits) for i in acct]))
     cand_g3 = float(np.mean([candidate_rows(host_events[i], r, 3, bits) for i in acct]))
     e_mean = float(np.mean(edges_per_event))
-    dom = max(phases_us, key=phases_us.get) if phases_us else "search_count"
-    alg_bytes = {"search_count": cand * 32.0, "search_write": cand * 32.0 + 12.0 * e_mean}.get(dom, cand * 32.0)
+    # dominant kernel = the search pass (one launch per step): candidate rows read + (j, d2) hit records written
+    dom = "search"
+    alg_bytes = cand * 32.0 + 8.0 * e_mean
     dom_us = phases_us.get(dom, float("nan"))
     achieved = alg_bytes / (dom_us * 1e-6) / 1e9 if dom_us and dom_us == dom_us else float("nan")
     traffic = None

@@ -79,6 +79,15 @@ int frnn_set_grid(int grid_dims, int grid_bits);
 void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits);
 
 /*
+ * Launch mode (process-global).  1 (default): a call on a non-default stream replays a cached CUDA
+ * graph of its kernels (keyed by every argument; built on first use, at most 128 kept, least
+ * recently used evicted) -- about 1 us per kernel boundary instead of about 3 us per stream launch.
+ * 0: kernels are launched one by one.  Calls on the legacy default stream, calls made while the
+ * caller is itself capturing the stream, and profiled calls always launch one by one.
+ */
+int frnn_set_graph_mode(int enabled);
+
+/*
  * The north_star 9-argument form.  Current device, legacy default stream, internally cached
  * workspace, output capacity assumed n*k_max edges (caller guarantees that much room, or at
  * least as many edges as the result has -- nothing is written beyond n*k_max).  SYNCHRONOUS:
@@ -135,8 +144,7 @@ int frnn_last_launch_count(void);
  * Per-phase device timing for bench.py's roofline line.  frnn_set_profiling(1) makes every later
  * frnn_build_ex/_batched call record one CUDA event after each phase of the path (on the call's
  * stream); frnn_get_profile waits for the LAST profiled call and writes the duration in ms of
- * each phase (memset, bin, scan_cells, scatter, search_count, scan_degrees, search_write,
- * sort_rows) into phase_ms[0..max_phases), returning the number of phases written or a negative
+ * each phase (memset, bin, scan_cells, scatter, search, emit) into phase_ms[0..max_phases), returning the number of phases written or a negative
  * status.  Process-global, not thread safe; leave it off when timing whole calls.
  */
 int frnn_set_profiling(int enabled);

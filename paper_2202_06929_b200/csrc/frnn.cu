@@ -1,10 +1,13 @@
 // frnn.cu -- host side of the C ABI declared in include/frnn.h (argument checks, workspace layout,
-// launch sequence).  No CPU fallback: every compute entry point needs a CUDA device.
+// launch sequence, CUDA-graph cache).  No CPU fallback: every compute entry point needs a CUDA device.
 #include "frnn_kernels.cuh"
 
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+
+#include <mutex>
+#include <vector>
 
 #include "../../include/frnn.h"
 
@@ -16,12 +19,12 @@ constexpr float kCellSlack = 1.0078125f;   // 1 + 2^-7, see cell_coord()
 constexpr size_t kAlign = 256;
 
 int g_force_dims = 0, g_force_bits = 0;
+int g_use_graph = 1;
 thread_local int t_launches = 0;
 
 // Optional per-phase CUDA-event timing (frnn_set_profiling): one event after every phase.
-constexpr int kPhases = 8;
-const char* const kPhaseNames[kPhases] = {"memset", "bin", "scan_cells", "scatter", "search_count", "scan_degrees",
-                                          "search_write", "sort_rows"};
+constexpr int kPhases = 6;
+const char* const kPhaseNames[kPhases] = {"memset", "bin", "scan_cells", "scatter", "search", "emit"};
 bool g_profiling = false;
 cudaEvent_t g_ev[kPhases + 1] = {};
 bool g_ev_valid = false;
@@ -44,30 +47,35 @@ GridChoice choose_grid(int64_t n_total, int n_events) {
     else g.dims = 5;
     int ev_bits = 0;
     while ((1ll << ev_bits) < n_events) ++ev_bits;
-    while (g.dims * g.bits + ev_bits > 31 && g.dims > 1) --g.dims;     // linear cell id is 32-bit
-    while (g.dims * g.bits + ev_bits > 31 && g.bits > 2) --g.bits;
+    while (g.dims * g.bits + ev_bits > 30 && g.dims > 1) --g.dims;     // padded table index stays below 2^31
+    while (g.dims * g.bits + ev_bits > 30 && g.bits > 2) --g.bits;
     return g;
 }
 
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    int64_t n_cells, tiles_a, tiles_b;
-    size_t off_cells, off_tiles_a, off_tiles_b, off_counters, zero_bytes;
-    size_t off_pcell, off_prank, off_spts, off_sidx, off_cnt, off_rowptr, off_evoff, off_segs, off_count;
+    int64_t n_cells, n_entries, emit_tiles;
+    int rows_per_block;
+    int64_t scan_blocks;
+    size_t off_cells, off_tiles, off_counters, zero_bytes;
+    size_t off_pcell, off_prank, off_spts, off_sidx, off_cnt, off_evoff, off_segs, off_hits;
     size_t total;
 };
 
 Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     Layout L;
     L.n_cells = static_cast<int64_t>(n_events) << (g.dims * g.bits);
-    L.tiles_a = (L.n_cells + kScanTile - 1) / kScanTile;
-    L.tiles_b = (n_total + kScanTile - 1) / kScanTile;
+    const int64_t row_len = (1ll << g.bits) + 1;
+    const int64_t n_rows = L.n_cells >> g.bits;
+    L.n_entries = n_rows * row_len;
+    L.rows_per_block = static_cast<int>(4096 / row_len > 0 ? 4096 / row_len : 1);
+    L.scan_blocks = (n_rows + L.rows_per_block - 1) / L.rows_per_block;
+    L.emit_tiles = (n_total + kEmitThreads - 1) / kEmitThreads;
     size_t o = 0;
-    L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_cells + 1) * 4);
-    L.off_tiles_a = o;  o = align_up(o + static_cast<size_t>(L.tiles_a) * 8);
-    L.off_tiles_b = o;  o = align_up(o + static_cast<size_t>(L.tiles_b > 0 ? L.tiles_b : 1) * 8);
-    L.off_counters = o; o = align_up(o + 64);
+    L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_entries + 1) * 4);
+    L.off_tiles = o;    o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8);
+    L.off_counters = o; o = align_up(o + 64);          // [0..7] cursor (u64), [8..11] emit ticket
     L.zero_bytes = o;
     const size_t n = static_cast<size_t>(n_total > 0 ? n_total : 1);
     const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
@@ -76,10 +84,9 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     L.off_spts = o;   o = align_up(o + n * 32);
     L.off_sidx = o;   o = align_up(o + n * 4);
     L.off_cnt = o;    o = align_up(o + n * 4);
-    L.off_rowptr = o; o = align_up(o + (n + 1) * 8);
     L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
     L.off_segs = o;   o = align_up(o + static_cast<size_t>(max_segs > 0 ? max_segs : 1) * sizeof(Segment));
-    L.off_count = o;  o = align_up(o + 64);
+    L.off_hits = o;   o = align_up(o + n * kSlot * sizeof(int2));
     L.total = o;
     return L;
 }
@@ -94,11 +101,11 @@ int num_sms() {
     return g_num_sms;
 }
 
-template <int G, int PASS>
+template <int G>
 cudaError_t launch_search(const SearchArgs& a, int64_t max_segs, cudaStream_t st) {
     static int blocks_per_sm = 0;
     if (!blocks_per_sm) {
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, search_kernel<G, PASS>, kSearchWarps * 32, 0) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, search_kernel<G>, kSearchWarps * 32, 0) != cudaSuccess ||
             blocks_per_sm < 1)
             blocks_per_sm = 1;
     }
@@ -106,16 +113,7 @@ cudaError_t launch_search(const SearchArgs& a, int64_t max_segs, cudaStream_t st
     const int64_t resident = static_cast<int64_t>(num_sms()) * blocks_per_sm;
     if (blocks > resident) blocks = resident;
     if (blocks < 1) blocks = 1;
-    search_kernel<G, PASS><<<static_cast<unsigned>(blocks), kSearchWarps * 32, 0, st>>>(a);
-    ++t_launches;
-    return cudaGetLastError();
-}
-
-template <int G>
-cudaError_t launch_bin(const float* pts, int64_t n, const int64_t* ev_off, int n_events, float inv_cell, int bits,
-                       uint32_t* cells, uint32_t* pcell, uint32_t* prank, cudaStream_t st) {
-    bin_kernel<G><<<static_cast<unsigned>((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(pts), n, ev_off, n_events,
-                                                                        inv_cell, bits, cells, pcell, prank);
+    search_kernel<G><<<static_cast<unsigned>(blocks), kSearchWarps * 32, 0, st>>>(a);
     ++t_launches;
     return cudaGetLastError();
 }
@@ -143,94 +141,170 @@ int check_common(const float* points, int64_t n, int dim, float r, int k_max, co
     return FRNN_OK;
 }
 
-// The whole path, enqueued on `st`.  ev_off_host has n_events+1 entries.
-int enqueue(const float* points, const int64_t* ev_off_host, int n_events, float r, int k_max,
-            int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t capacity,
-            int64_t* out_count, int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
-            void* workspace, size_t workspace_bytes, cudaStream_t st) {
-    t_launches = 0;
-    const int64_t n_total = ev_off_host[n_events];
-    if (n_total == 0) {                       // nothing to search: zero the outputs and leave
-        if (out_count) { CK(cudaMemsetAsync(out_count, 0, 8, st)); ++t_launches; }
-        if (out_edge_offsets) { CK(cudaMemsetAsync(out_edge_offsets, 0, 8 * static_cast<size_t>(n_events + 1), st)); ++t_launches; }
-        if (out_row_ptr) { CK(cudaMemsetAsync(out_row_ptr, 0, 8, st)); ++t_launches; }
-        CK(cudaMemsetAsync(out_status, 0, 4, st)); ++t_launches;
-        return FRNN_OK;
+struct Call {                 // everything that determines the enqueued work (also the graph-cache key)
+    const float* points;
+    int n_events;
+    float r;
+    int k_max;
+    int32_t* out_src;
+    int32_t* out_dst;
+    float* out_d2;
+    int64_t capacity;
+    int64_t* out_count;
+    int64_t* out_edge_offsets;
+    int32_t* out_status;
+    int64_t* out_row_ptr;
+    void* workspace;
+    int grid_dims, grid_bits;
+    std::vector<int64_t> ev_off;
+    bool operator==(const Call& o) const {
+        return points == o.points && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
+               out_dst == o.out_dst && out_d2 == o.out_d2 && capacity == o.capacity && out_count == o.out_count &&
+               out_edge_offsets == o.out_edge_offsets && out_status == o.out_status && out_row_ptr == o.out_row_ptr &&
+               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off;
     }
-    const GridChoice g = choose_grid(n_total, n_events);
-    const Layout L = make_layout(n_total, n_events, g);
-    if (!workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
-    if (reinterpret_cast<uintptr_t>(workspace) % kAlign) return FRNN_ERR_INVALID_ARG;
-    char* ws = static_cast<char*>(workspace);
+};
+
+// The whole path, enqueued kernel by kernel on `st`.
+int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
+    const int64_t n_total = c.ev_off[c.n_events];
+    char* ws = static_cast<char*>(c.workspace);
     uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
-    uint64_t* tiles_a = reinterpret_cast<uint64_t*>(ws + L.off_tiles_a);
-    uint64_t* tiles_b = reinterpret_cast<uint64_t*>(ws + L.off_tiles_b);
-    uint32_t* counters = reinterpret_cast<uint32_t*>(ws + L.off_counters);   // [0] ticket A, [1] ticket B, [2] n_segs
+    uint64_t* tiles = reinterpret_cast<uint64_t*>(ws + L.off_tiles);
+    unsigned long long* cursor = reinterpret_cast<unsigned long long*>(ws + L.off_counters);
+    uint32_t* ticket = reinterpret_cast<uint32_t*>(ws + L.off_counters + 8);
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
     int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
-    int64_t* row_ptr = out_row_ptr ? out_row_ptr : reinterpret_cast<int64_t*>(ws + L.off_rowptr);
     int64_t* ev_off = reinterpret_cast<int64_t*>(ws + L.off_evoff);
     Segment* segs = reinterpret_cast<Segment*>(ws + L.off_segs);
+    int2* hits = reinterpret_cast<int2*>(ws + L.off_hits);
+    const float4* pts = reinterpret_cast<const float4*>(c.points);
+    const int G = c.grid_dims, bits = c.grid_bits;
 
-    const float r2 = r * r;                                   // R2: fl32(r*r), once, on the host
-    const float cell_side = fmaxf(r * kCellSlack, 1e-30f);
+    const float r2 = c.r * c.r;                               // R2: fl32(r*r), once, on the host
+    const float cell_side = fmaxf(c.r * kCellSlack, 1e-30f);
     const float inv_cell = 1.0f / cell_side;
 
     mark(-1, st);
     CK(cudaMemsetAsync(ws, 0, L.zero_bytes, st)); ++t_launches;
     // Event offsets reach the device as kernel arguments (no pageable-memory copy, which would
     // synchronise the host with the stream); a single event needs none (base 0).
-    if (n_events > 1) {
-        for (int first = 0; first <= n_events; first += OffsetChunk::kN) {
-            OffsetChunk c;
-            c.first = first;
-            c.count = (n_events + 1 - first) < OffsetChunk::kN ? (n_events + 1 - first) : OffsetChunk::kN;
-            for (int k = 0; k < c.count; ++k) c.v[k] = ev_off_host[first + k];
-            set_offsets_kernel<<<1, OffsetChunk::kN, 0, st>>>(c, ev_off);
+    if (c.n_events > 1) {
+        for (int first = 0; first <= c.n_events; first += OffsetChunk::kN) {
+            OffsetChunk ch;
+            ch.first = first;
+            ch.count = (c.n_events + 1 - first) < OffsetChunk::kN ? (c.n_events + 1 - first) : OffsetChunk::kN;
+            for (int k = 0; k < ch.count; ++k) ch.v[k] = c.ev_off[first + k];
+            set_offsets_kernel<<<1, OffsetChunk::kN, 0, st>>>(ch, ev_off);
             ++t_launches; CK(cudaGetLastError());
         }
     } else {
         ev_off = nullptr;
     }
-
     mark(0, st);
-    FRNN_DISPATCH_G(g.dims, CK(launch_bin<GG>(points, n_total, ev_off, n_events, inv_cell, g.bits, cells, pcell, prank, st)));
+    const unsigned row_blocks = static_cast<unsigned>((n_total + 255) / 256);
+    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank)));
+    ++t_launches; CK(cudaGetLastError());
     mark(1, st);
-
-    scan_kernel<CellScan><<<static_cast<unsigned>(L.tiles_a), kScanThreads, 0, st>>>(CellScan{cells, segs, counters + 2}, L.n_cells,
-                                                                                   tiles_a, counters + 0);
+    FRNN_DISPATCH_G(G, (cell_scan_kernel<GG><<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries,
+                                                                                                           L.rows_per_block, bits, segs, cursor)));
     ++t_launches; CK(cudaGetLastError());
     mark(2, st);
-
-    scatter_kernel<<<static_cast<unsigned>((n_total + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float4*>(points), n_total, cells,
-                                                                               pcell, prank, spts, sidx);
+    scatter_kernel<<<row_blocks, 256, 0, st>>>(pts, n_total, cells, pcell, prank, spts, sidx);
     ++t_launches; CK(cudaGetLastError());
     mark(3, st);
 
-    SearchArgs a;
-    a.spts = spts; a.sidx = sidx; a.cell_start = cells; a.segs = segs; a.n_segs = counters + 2; a.ev_off = ev_off;
-    a.cnt = cnt; a.row_ptr = row_ptr; a.out_src = out_src; a.out_dst = out_dst; a.out_d2 = out_d2;
-    a.capacity = capacity; a.r2 = r2; a.bits = g.bits; a.k_max = static_cast<uint32_t>(k_max);
+    SearchArgs sa;
+    sa.spts = spts; sa.sidx = sidx; sa.cell_start = cells; sa.segs = segs; sa.cursor = cursor; sa.cnt = cnt; sa.hits = hits;
+    sa.r2 = r2; sa.bits = bits;
     const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
-
-    FRNN_DISPATCH_G(g.dims, CK((launch_search<GG, 0>(a, max_segs, st))));
+    FRNN_DISPATCH_G(G, CK((launch_search<GG>(sa, max_segs, st))));
     mark(4, st);
 
-    scan_kernel<DegreeScan><<<static_cast<unsigned>(L.tiles_b), kScanThreads, 0, st>>>(DegreeScan{cnt, row_ptr, static_cast<uint32_t>(k_max)},
-                                                                                     n_total, tiles_b, counters + 1);
+    EmitArgs ea;
+    ea.pts = pts; ea.spts = spts; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
+    ea.n_events = c.n_events; ea.n_total = n_total; ea.tile_state = tiles; ea.ticket = ticket; ea.row_ptr = c.out_row_ptr;
+    ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
+    ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
+    ea.k_max = static_cast<uint32_t>(c.k_max);
+    FRNN_DISPATCH_G(G, (emit_kernel<GG><<<static_cast<unsigned>(L.emit_tiles), kEmitThreads, 0, st>>>(ea)));
     ++t_launches; CK(cudaGetLastError());
     mark(5, st);
+    return FRNN_OK;
+}
 
-    FRNN_DISPATCH_G(g.dims, CK((launch_search<GG, 1>(a, max_segs, st))));
-    mark(6, st);
+// ---- CUDA-graph cache: the same call (same pointers, sizes, parameters) replays one instantiated
+// graph, which costs ~1 us per kernel boundary instead of ~3 us per stream launch (profiles/).
+struct CachedGraph { Call key; cudaGraphExec_t exec; int launches; uint64_t stamp; };
+std::vector<CachedGraph> g_graphs;
+std::mutex g_graph_mutex;
+uint64_t g_stamp = 0;
+constexpr size_t kMaxGraphs = 128;
 
-    sort_rows_kernel<<<static_cast<unsigned>((n_total + 255) / 256), 256, 0, st>>>(row_ptr, n_total, capacity, out_dst, out_d2, ev_off,
-                                                                                 n_events, out_count, out_edge_offsets, out_status);
-    ++t_launches; CK(cudaGetLastError());
-    mark(7, st);
+int run_call(const Call& c, cudaStream_t st) {
+    t_launches = 0;
+    const int64_t n_total = c.ev_off[c.n_events];
+    if (n_total == 0) {                       // nothing to search: zero the outputs and leave
+        if (c.out_count) { CK(cudaMemsetAsync(c.out_count, 0, 8, st)); ++t_launches; }
+        if (c.out_edge_offsets) { CK(cudaMemsetAsync(c.out_edge_offsets, 0, 8 * static_cast<size_t>(c.n_events + 1), st)); ++t_launches; }
+        if (c.out_row_ptr) { CK(cudaMemsetAsync(c.out_row_ptr, 0, 8, st)); ++t_launches; }
+        CK(cudaMemsetAsync(c.out_status, 0, 4, st)); ++t_launches;
+        return FRNN_OK;
+    }
+    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits});
+    bool graph_ok = g_use_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
+    if (graph_ok) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) graph_ok = false;   // caller is capturing: just enqueue
+    }
+    if (!graph_ok) return enqueue(c, L, st);
+
+    std::lock_guard<std::mutex> lock(g_graph_mutex);
+    for (auto& g : g_graphs) {
+        if (g.key == c) {
+            g.stamp = ++g_stamp;
+            t_launches = g.launches;
+            CK(cudaGraphLaunch(g.exec, st));
+            return FRNN_OK;
+        }
+    }
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return enqueue(c, L, st); }
+    const int rc = enqueue(c, L, st);
+    const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+    if (rc != FRNN_OK || ce != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return rc != FRNN_OK ? rc : FRNN_ERR_CUDA;
+    }
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ie = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ie != cudaSuccess) { cudaGetLastError(); return FRNN_ERR_CUDA; }
+    if (g_graphs.size() >= kMaxGraphs) {      // evict the least recently used
+        size_t victim = 0;
+        for (size_t k = 1; k < g_graphs.size(); ++k)
+            if (g_graphs[k].stamp < g_graphs[victim].stamp) victim = k;
+        cudaGraphExecDestroy(g_graphs[victim].exec);
+        g_graphs.erase(g_graphs.begin() + victim);
+    }
+    g_graphs.push_back(CachedGraph{c, exec, t_launches, ++g_stamp});
+    CK(cudaGraphLaunch(exec, st));
+    return FRNN_OK;
+}
+
+int prepare(Call& c, size_t workspace_bytes) {
+    const int64_t n_total = c.ev_off[c.n_events];
+    const GridChoice g = choose_grid(n_total, c.n_events);
+    c.grid_dims = g.dims;
+    c.grid_bits = g.bits;
+    if (n_total == 0) return FRNN_OK;
+    const Layout L = make_layout(n_total, c.n_events, g);
+    if (!c.workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
+    if (reinterpret_cast<uintptr_t>(c.workspace) % kAlign) return FRNN_ERR_INVALID_ARG;
     return FRNN_OK;
 }
 
@@ -240,6 +314,7 @@ struct Cache {
     void* misc = nullptr;                       // count (8) + status (4)
     void* pts = nullptr; size_t pts_bytes = 0;
     void* edges = nullptr; size_t edge_cap = 0; // src | dst | d2, edge_cap each
+    cudaStream_t stream = nullptr;              // non-default stream so the graph path applies
 } g_cache;
 
 int ensure(void** p, size_t* have, size_t need) {
@@ -251,11 +326,16 @@ int ensure(void** p, size_t* have, size_t need) {
     return FRNN_OK;
 }
 
+int ensure_stream() {
+    if (!g_cache.stream && cudaStreamCreateWithFlags(&g_cache.stream, cudaStreamNonBlocking) != cudaSuccess) return FRNN_ERR_CUDA;
+    return FRNN_OK;
+}
+
 }  // namespace
 
 extern "C" {
 
-int frnn_version(void) { return 100; }   // 0.1.0
+int frnn_version(void) { return 200; }   // 0.2.0
 
 const char* frnn_status_string(int status) {
     switch (status) {
@@ -287,6 +367,11 @@ void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits
     if (grid_bits) *grid_bits = g.bits;
 }
 
+int frnn_set_graph_mode(int enabled) {
+    g_use_graph = enabled != 0;
+    return FRNN_OK;
+}
+
 int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
                   int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                   int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
@@ -294,9 +379,9 @@ int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
     int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
     if (rc != FRNN_OK) return rc;
     if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
-    const int64_t ev_off[2] = {0, n};
-    return enqueue(points, ev_off, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status,
-                   out_row_ptr, workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+    Call c{points, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
+    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
+    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int frnn_build_batched(const float* points, const int64_t* event_offsets, int n_events, int dim, float r, int k_max,
@@ -309,8 +394,10 @@ int frnn_build_batched(const float* points, const int64_t* event_offsets, int n_
     int rc = check_common(points, event_offsets[n_events], dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
     if (rc != FRNN_OK) return rc;
     if (!out_edge_offsets || !out_status) return FRNN_ERR_INVALID_ARG;
-    return enqueue(points, event_offsets, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets,
-                   out_status, out_row_ptr, workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+    Call c{points, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets, out_status, out_row_ptr,
+           workspace, 0, 0, std::vector<int64_t>(event_offsets, event_offsets + n_events + 1)};
+    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
+    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
@@ -326,7 +413,7 @@ int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
     int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
     int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
     rc = frnn_build_ex(points, n, dim, r, k_max, out_src, out_dst, out_d2, cap, d_count, d_status, nullptr, g_cache.ws,
-                       g_cache.ws_bytes, nullptr);
+                       g_cache.ws_bytes, nullptr);       // legacy default stream, as documented
     if (rc != FRNN_OK) return rc;
     int32_t h_status = 0;
     CK(cudaMemcpy(out_count, d_count, 8, cudaMemcpyDeviceToHost));
@@ -342,6 +429,7 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     const size_t need = frnn_workspace_bytes(n, 1, dim, k_max);
     size_t misc_have = g_cache.misc ? 64 : 0;
     size_t edge_bytes = g_cache.edge_cap * 12;
+    if ((rc = ensure_stream()) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.ws, &g_cache.ws_bytes, need)) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.misc, &misc_have, 64)) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.pts, &g_cache.pts_bytes, static_cast<size_t>(n > 0 ? n : 1) * 32)) != FRNN_OK) return rc;
@@ -349,23 +437,25 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
         if ((rc = ensure(&g_cache.edges, &edge_bytes, static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1) * 12)) != FRNN_OK) return rc;
         g_cache.edge_cap = static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1);
     }
+    cudaStream_t st = g_cache.stream;
     int32_t* d_src = static_cast<int32_t*>(g_cache.edges);
     int32_t* d_dst = d_src + g_cache.edge_cap;
     float* d_d2 = reinterpret_cast<float*>(d_dst + g_cache.edge_cap);
     int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
     int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
-    if (n > 0) CK(cudaMemcpyAsync(g_cache.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, nullptr));
+    if (n > 0) CK(cudaMemcpyAsync(g_cache.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, st));
     rc = frnn_build_ex(static_cast<const float*>(g_cache.pts), n, dim, r, k_max, d_src, d_dst, d_d2, edge_capacity, d_count, d_status,
-                       nullptr, g_cache.ws, g_cache.ws_bytes, nullptr);
+                       nullptr, g_cache.ws, g_cache.ws_bytes, st);
     if (rc != FRNN_OK) return rc;
-    CK(cudaMemcpy(out_count, d_count, 8, cudaMemcpyDeviceToHost));
+    CK(cudaMemcpyAsync(out_count, d_count, 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
     if (*out_count > edge_capacity) return FRNN_ERR_CAPACITY;
     const size_t e = static_cast<size_t>(*out_count);
     if (e) {
-        CK(cudaMemcpyAsync(out_src, d_src, e * 4, cudaMemcpyDeviceToHost, nullptr));
-        CK(cudaMemcpyAsync(out_dst, d_dst, e * 4, cudaMemcpyDeviceToHost, nullptr));
-        CK(cudaMemcpyAsync(out_d2, d_d2, e * 4, cudaMemcpyDeviceToHost, nullptr));
-        CK(cudaStreamSynchronize(nullptr));
+        CK(cudaMemcpyAsync(out_src, d_src, e * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(out_dst, d_dst, e * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(out_d2, d_d2, e * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
     }
     return FRNN_OK;
 }
@@ -394,10 +484,16 @@ int frnn_get_profile(float* phase_ms, int max_phases) {
 const char* frnn_phase_name(int phase) { return (phase >= 0 && phase < kPhases) ? kPhaseNames[phase] : ""; }
 
 void frnn_release_cached(void) {
+    {
+        std::lock_guard<std::mutex> lock(g_graph_mutex);
+        for (auto& g : g_graphs) cudaGraphExecDestroy(g.exec);
+        g_graphs.clear();
+    }
     if (g_cache.ws) cudaFree(g_cache.ws);
     if (g_cache.misc) cudaFree(g_cache.misc);
     if (g_cache.pts) cudaFree(g_cache.pts);
     if (g_cache.edges) cudaFree(g_cache.edges);
+    if (g_cache.stream) cudaStreamDestroy(g_cache.stream);
     g_cache = Cache{};
 }
 

@@ -1,13 +1,15 @@
 // frnn_kernels.cuh -- device code of the B200 FRNN path (sm_100a).  Product code: shares nothing
 // with oracle/.  Steps S2..S10 of SURVEY.md section 8(a); design notes in DESIGN.md section 6.
 //
-//   bin_kernel      S2  cell index on a toroidal grid over the first G coordinates + histogram
-//   scan_kernel     S3/S9 single-pass decoupled look-back scan (cells -> cell_start + segment list;
-//                   capped degrees -> CSR row_ptr)
-//   scatter_kernel  S4  counting-sort scatter into the cell-ordered copy
-//   search_kernel   S5..S8,S10 one warp per occupied cell ("segment"): neighbour runs are
-//                   flattened across lanes, every lane evaluates whole 8-term FMA chains
-//   sort_rows_kernel S10 per-row ordering by dst + call epilogue (count, status, edge offsets)
+//   bin_kernel      S2     cell index on a toroidal grid over the first G coordinates + histogram
+//   cell_scan_kernel S3    cell starts + list of occupied cells ("segments"); blocks take their base
+//                          from one atomic (no inter-block wait), rows of the table are padded so a
+//                          run never needs the next block's start
+//   scatter_kernel  S4     counting-sort scatter into the cell-ordered copy
+//   search_kernel   S5-S7  ONE pass: a warp per occupied cell, neighbour runs flattened across
+//                          lanes, whole 8-term FMA chains per lane; hits go to a per-row slot buffer
+//   emit_kernel     S8-S10 degree scan (decoupled look-back) fused with the per-row ordering by dst
+//                          and the compaction into the (src,dst)-sorted COO; exact K-cap selection
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -24,6 +26,11 @@ constexpr unsigned kFull = 0xffffffffu;
 // monotone, so points beyond +-2^15 cells only pile up in the boundary cells (slower, still exact).
 // The modulo (toroidal wrap) only ever ADDS candidates: far-apart points may share a cell, the
 // full-D distance test rejects them.
+//
+// Linear cell id  lin = (((event << bits | c0) << bits | c1) ...) << bits | c_last.
+// Table index     pid = lin + (lin >> bits): every row of 2^bits cells along the last coordinate
+// is followed by one padding entry whose count is 0, so after the exclusive scan it holds the END
+// of the row and  [start[pid(lo)], start[pid(hi) + 1])  is a valid run for any lo <= hi in the row.
 // ------------------------------------------------------------------------------------------------
 constexpr float kCoordClamp = 32768.0f;
 
@@ -32,6 +39,18 @@ __device__ __forceinline__ uint32_t cell_coord(float x, float inv_cell, uint32_t
     a = fminf(fmaxf(a, -kCoordClamp), kCoordClamp);   // NaN -> -clamp: never out of bounds
     return static_cast<uint32_t>(__float2int_rd(a)) & mask;
 }
+
+template <int G>
+__device__ __forceinline__ uint32_t cell_of_point(const float4& a, const float4& b, uint32_t event, float inv_cell, int bits) {
+    const uint32_t mask = (1u << bits) - 1u;
+    const float x[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+    uint32_t lin = event;
+#pragma unroll
+    for (int d = 0; d < G; ++d) lin = (lin << bits) | cell_coord(x[d], inv_cell, mask);
+    return lin;
+}
+
+__device__ __forceinline__ uint32_t padded(uint32_t lin, int bits) { return lin + (lin >> bits); }
 
 // DESIGN.md R3: the pinned fp32 order.  Explicit rounding intrinsics: nvcc may not contract,
 // reassociate or reorder them.  Each lane runs the whole chain for one (query, candidate) pair.
@@ -79,16 +98,13 @@ __global__ void __launch_bounds__(256) bin_kernel(const float4* __restrict__ pts
                                                   uint32_t* __restrict__ pcell, uint32_t* __restrict__ prank) {
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i >= n_total) return;
-    const uint32_t mask = (1u << bits) - 1u;
     const float4 a = pts[2 * i];
     float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
     if (G > 4) b = pts[2 * i + 1];
-    const float x[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-    uint32_t lin = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
-#pragma unroll
-    for (int d = 0; d < G; ++d) lin = (lin << bits) | cell_coord(x[d], inv_cell, mask);
-    pcell[i] = lin;
-    prank[i] = atomicAdd(&cell_count[lin], 1u);
+    const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
+    const uint32_t pid = padded(cell_of_point<G>(a, b, ev, inv_cell, bits), bits);
+    pcell[i] = pid;
+    prank[i] = atomicAdd(&cell_count[pid], 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -110,103 +126,395 @@ __global__ void __launch_bounds__(256) scatter_kernel(const float4* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------------
-// S3 / S9: single-pass exclusive scan with decoupled look-back.  One 64-bit descriptor per tile:
-// [63:62] flag (0 = not ready, 1 = tile aggregate, 2 = inclusive prefix), [61:0] value.
-// Tiles take their index from an atomic ticket, so a tile only ever waits on tiles that have
-// already started (no dependence on block scheduling order).
+// S3: cell starts.  Each block owns a few WHOLE padded rows of the table (about 4096 entries),
+// computes its total, reserves its range of the cell-ordered copy with ONE 64-bit atomicAdd that
+// packs (occupied cells << 32 | points), then scans its rows in strips of 1024.  Blocks land in
+// arrival order: no inter-block wait, and since a run only ever reads start[lo] and start[hi+1] of
+// one row (the padding entry holds the row's end) nothing depends on the order of the blocks.
+// The block also appends its occupied cells to the segment list (same atomic).
 // ------------------------------------------------------------------------------------------------
-constexpr int kScanThreads = 512;
-constexpr int kScanItems = 8;
-constexpr int kScanTile = kScanThreads * kScanItems;
-constexpr uint64_t kFlagA = 1ull << 62, kFlagP = 2ull << 62, kValMask = (1ull << 62) - 1;
-
-__device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) {
-    uint64_t v;
-    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p));
-    return v;
-}
-__device__ __forceinline__ void st_volatile_u64(uint64_t* p, uint64_t v) {
-    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
-struct Segment {          // one occupied cell: the unit of work of the search kernels
+struct Segment {          // one occupied cell: the unit of work of the search kernel
     uint32_t cell;        // linear cell id (event index in the high bits)
     uint32_t start;       // first slot in the cell-ordered copy
     uint32_t len;         // points in the cell
-    uint32_t pad;
+    uint32_t interior;    // 1 if no coordinate of the cell is 0 or 2^bits-1 (no wrap among its neighbours)
 };
 
-// Policy A: cell histogram -> cell_start (in place) + compacted list of occupied cells.
-// Value packs (occupied cells so far) << 32 | (points so far).
-struct CellScan {
-    uint32_t* cells;          // in: counts, out: exclusive starts; [n] = total
-    Segment* segs;
-    uint32_t* n_segs;
-    __device__ __forceinline__ uint64_t value(uint32_t v) const { return (static_cast<uint64_t>(v != 0) << 32) | v; }
-    __device__ __forceinline__ uint32_t load(int64_t i) const { return cells[i]; }
-    __device__ __forceinline__ void store(int64_t i, uint32_t v, uint64_t excl) const {
-        cells[i] = static_cast<uint32_t>(excl);
-        if (v) segs[excl >> 32] = Segment{static_cast<uint32_t>(i), static_cast<uint32_t>(excl), v, 0u};
+constexpr int kCellThreads = 1024;
+
+// A block owns `rows_per_block` whole padded rows, i.e. rows_per_block * (2^bits + 1) entries.
+template <int G>
+__global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __restrict__ cells, int64_t n_entries, int rows_per_block,
+                                                                 int bits, Segment* __restrict__ segs,
+                                                                 unsigned long long* __restrict__ cursor) {
+    __shared__ uint64_t s_warp[kCellThreads / 32];
+    __shared__ uint64_t s_base;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int row_len = (1 << bits) + 1;
+    const int64_t blk_entries = static_cast<int64_t>(rows_per_block) * row_len;
+    const int64_t blk_base = static_cast<int64_t>(blockIdx.x) * blk_entries;
+    const int64_t blk_end = min(blk_base + blk_entries, n_entries);
+    const uint32_t mask = (1u << bits) - 1u;
+    uint64_t carry = 0;                                   // (occupied << 32 | points) of earlier strips
+    // pass 1: block total (so that ONE atomic reserves the block's range), strip by strip
+    uint64_t tsum = 0;
+    for (int64_t i = blk_base + threadIdx.x; i < blk_end; i += kCellThreads) {
+        const uint32_t v = cells[i];
+        tsum += (static_cast<uint64_t>(v != 0) << 32) | v;
     }
-    __device__ __forceinline__ void finish(int64_t n, uint64_t total) const {
-        cells[n] = static_cast<uint32_t>(total);
-        *n_segs = static_cast<uint32_t>(total >> 32);
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) tsum += __shfl_xor_sync(kFull, tsum, o);
+    if (lane == 0) s_warp[warp] = tsum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint64_t t = 0;
+        for (int w = 0; w < kCellThreads / 32; ++w) t += s_warp[w];
+        s_base = t ? atomicAdd(cursor, static_cast<unsigned long long>(t)) : 0ull;
     }
+    __syncthreads();
+    carry = s_base;
+    __syncthreads();
+    // pass 2: exclusive scan strip by strip (the strip's counts are L1/L2 hits now)
+    for (int64_t s0 = blk_base; s0 < blk_end; s0 += kCellThreads) {
+        const int64_t i = s0 + threadIdx.x;
+        const uint32_t v = i < blk_end ? cells[i] : 0u;
+        const uint64_t val = (static_cast<uint64_t>(v != 0) << 32) | v;
+        uint64_t incl = val;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint64_t t = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        uint64_t wexcl = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < kCellThreads / 32; ++w) {
+            const uint64_t t = s_warp[w];
+            if (w < warp) wexcl += t;
+            total += t;
+        }
+        const uint64_t excl = carry + wexcl + (incl - val);
+        if (i < blk_end) {
+            cells[i] = static_cast<uint32_t>(excl);
+            if (v) {
+                // table index -> linear id: remove the padding entries (row = i / row_len)
+                const uint32_t row = static_cast<uint32_t>(i / row_len);
+                const uint32_t lin = static_cast<uint32_t>(i) - row;
+                bool interior = true;
+#pragma unroll
+                for (int d = 0; d < G; ++d) {
+                    const uint32_t c = (lin >> (d * bits)) & mask;
+                    interior = interior && c != 0u && c != mask;
+                }
+                segs[excl >> 32] = Segment{lin, static_cast<uint32_t>(excl), v, interior ? 1u : 0u};
+            }
+        }
+        carry += total;
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S5: neighbour-cell enumeration for one occupied cell.  The last binned coordinate is the
+// fastest-varying one in the linear cell id, so its three adjacent cells are ONE contiguous run of
+// the cell-ordered copy: 3^G cells = 3^(G-1) runs.  Up to 27 runs live in lanes (one per lane);
+// G > 4 loops over 3^(G-4) run groups.  Interior cells (the common case) reach a neighbour row by
+// adding a per-lane constant to the cell id; cells on a face of the toroidal grid take the general
+// path with wrapped coordinates and, for the last coordinate, a second "piece".
+//
+// Flattening: an inclusive warp scan of the run lengths gives every run its offset E_k in the
+// flattened candidate list.  For the chunk [b, b+32) each lane needs the run with the largest
+// E_k <= b + lane: (number of non-empty runs with E_k <= b) + popc of the marks of runs starting
+// inside (b, b+lane] -- one REDUX.OR, one ballot and two popc instead of a per-lane search.
+// f(slot_or_minus1) is called once per chunk with one candidate slot per lane (-1 = no candidate).
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int pow3(int e) { return e <= 0 ? 1 : 3 * pow3(e - 1); }
+
+template <int G>
+struct Neigh {
+    static constexpr int LD = (G - 1 < 3) ? (G - 1) : 3;     // coordinates enumerated across lanes
+    static constexpr int RL = pow3(LD);                      // runs per group (<= 27)
+    static constexpr int GD = G - 1 - LD;                    // coordinates enumerated by the group loop
+    static constexpr int NG = pow3(GD);
 };
 
-// Policy B: uncapped per-row counts -> CSR row_ptr of min(count, k_max)  (S9).
-struct DegreeScan {
+// signed cell-id offset of this lane's neighbour row (interior cells only)
+template <int G>
+__device__ __forceinline__ int lane_row_delta(int lane, int bits) {
+    int kk = lane, delta = 0;
+#pragma unroll
+    for (int d = Neigh<G>::GD; d < G - 1; ++d) {
+        const int o = kk % 3 - 1;
+        kk /= 3;
+        delta += o * (1 << ((G - 1 - d) * bits));
+    }
+    return delta;
+}
+
+template <int G, class F>
+__device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, bool interior, int bits, int lane_delta,
+                                                         const uint32_t* __restrict__ cell_start, int* s_delta,
+                                                         int lane, F&& f) {
+    using N = Neigh<G>;
+    const uint32_t mask = (1u << bits) - 1u;
+    const uint32_t c_last = cell & mask;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const bool edge_lo = c_last == 0u, edge_hi = c_last == mask;
+    const int n_pieces = (!interior && (edge_lo || edge_hi)) ? 2 : 1;
+    for (int grp = 0; grp < N::NG; ++grp) {
+        uint32_t row;                                        // padded table index of the neighbour row's cell 0
+        if (interior) {
+            int gdelta = 0, gg = grp;
+#pragma unroll
+            for (int d = 0; d < N::GD; ++d) { gdelta += (gg % 3 - 1) * (1 << ((G - 1 - d) * bits)); gg /= 3; }
+            row = padded((cell & ~mask) + static_cast<uint32_t>(lane_delta + gdelta), bits);
+        } else {
+            uint32_t base = cell >> (G * bits);
+            int kk = lane, gg = grp;
+#pragma unroll
+            for (int d = 0; d < G - 1; ++d) {
+                int o;
+                if (d < N::GD) { o = gg % 3 - 1; gg /= 3; } else { o = kk % 3 - 1; kk /= 3; }
+                const uint32_t cd = (cell >> ((G - 1 - d) * bits)) & mask;
+                base = (base << bits) | ((cd + static_cast<uint32_t>(o)) & mask);
+            }
+            row = padded(base << bits, bits);
+        }
+        for (int piece = 0; piece < n_pieces; ++piece) {
+            uint32_t lo, hi;
+            if (piece == 0) { lo = edge_lo ? 0u : c_last - 1u; hi = edge_hi ? mask : c_last + 1u; }
+            else            { lo = hi = edge_lo ? mask : 0u; }
+            uint32_t s = 0, e = 0;
+            if (lane < N::RL) { s = cell_start[row + lo]; e = cell_start[row + hi + 1u]; }
+            const int len = static_cast<int>(e - s);
+            int incl = len;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(kFull, incl, o);
+                if (lane >= o) incl += t;
+            }
+            const int total = __shfl_sync(kFull, incl, 31);
+            if (total == 0) continue;
+            const int excl = incl - len;
+            const uint32_t nz = __ballot_sync(kFull, len > 0);
+            __syncwarp();
+            if (len > 0) s_delta[__popc(nz & lt_mask)] = static_cast<int>(s) - excl;   // slot = t + delta within the run
+            __syncwarp();
+            for (int b = 0; b < total; b += 32) {
+                const int rel = excl - b;                                // where this run starts relative to the chunk
+                const uint32_t mark = (len > 0 && rel > 0 && rel < 32) ? (1u << rel) : 0u;
+                const uint32_t marks = __reduce_or_sync(kFull, mark);
+                const int before = __popc(__ballot_sync(kFull, len > 0 && rel <= 0));
+                const int ord = before - 1 + __popc(marks & ((2u << lane) - 1u));
+                const int t = b + lane;
+                const int slot = t < total ? t + s_delta[ord] : -1;
+                f(slot);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S6/S7: the single search pass.  One warp per segment (occupied cell), persistent grid-stride
+// over the segment list.  Queries = the cell's points (<= 32 per pass) staged in shared memory and
+// read back as broadcasts; candidates = one per lane per chunk (2 x 128-bit loads of the 32-byte
+// row).  Lane q keeps the running hit count of query q.  Every hit (j, d2) is appended to the
+// query's slot buffer hits[row * kSlot + pos] (pos < kSlot); the count keeps running beyond kSlot,
+// which tells emit_kernel to resolve that row by recomputation.
+// ------------------------------------------------------------------------------------------------
+constexpr int kSearchWarps = 8;
+constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
+
+struct SearchArgs {
+    const float4* spts;
+    const int32_t* sidx;          // slot -> global row index
+    const uint32_t* cell_start;
+    const Segment* segs;
+    const unsigned long long* cursor;   // high 32 bits = number of segments
+    uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index
+    int2* hits;                   // [n_total * kSlot] (j global, d2 bits)
+    float r2;
+    int bits;
+};
+
+template <int G>
+__global__ void __launch_bounds__(kSearchWarps * 32) search_kernel(SearchArgs a) {
+    __shared__ float4 s_q[kSearchWarps][64];
+    __shared__ int s_delta[kSearchWarps][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const uint32_t n_segs = static_cast<uint32_t>(*a.cursor >> 32);
+    const uint32_t stride = gridDim.x * kSearchWarps;
+    const int lane_delta = lane_row_delta<G>(lane, a.bits);
+    float4* q = s_q[warp];
+    const float inf = __int_as_float(0x7f800000);
+    for (uint32_t sg = blockIdx.x * kSearchWarps + warp; sg < n_segs; sg += stride) {
+        const Segment seg = a.segs[sg];
+        for (uint32_t q0 = 0; q0 < seg.len; q0 += 32) {
+            const int nq = min(32u, seg.len - q0);
+            const uint32_t first_slot = seg.start + q0;
+            const bool has = lane < nq;
+            int32_t my_row = 0;
+            uint32_t my_cnt = 0;
+            __syncwarp();
+            if (has) {
+                q[2 * lane] = a.spts[2 * static_cast<int64_t>(first_slot + lane)];
+                q[2 * lane + 1] = a.spts[2 * static_cast<int64_t>(first_slot + lane) + 1];
+                my_row = a.sidx[first_slot + lane];
+            }
+            __syncwarp();
+            for_each_candidate_chunk<G>(seg.cell, seg.interior != 0u, a.bits, lane_delta, a.cell_start, s_delta[warp], lane,
+                                        [&](int cslot) {
+                float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);   // no candidate: d2 = inf
+                int32_t cj = 0;
+                if (cslot >= 0) {
+                    ca = a.spts[2 * static_cast<int64_t>(cslot)];
+                    cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
+                    cj = a.sidx[cslot];
+                }
+                const int self_q = cslot - static_cast<int>(first_slot);   // the query this candidate IS (if in [0, nq))
+                for (int qi = 0; qi < nq; ++qi) {
+                    const float d2 = d2_pinned(q[2 * qi], q[2 * qi + 1], ca, cb);
+                    const bool hit = d2 <= a.r2 && self_q != qi;
+                    const uint32_t m = __ballot_sync(kFull, hit);
+                    if (m) {
+                        const uint32_t base = __shfl_sync(kFull, my_cnt, qi);
+                        const int32_t row = __shfl_sync(kFull, my_row, qi);
+                        if (hit) {
+                            const uint32_t pos = base + __popc(m & lt_mask);
+                            if (pos < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + pos] = make_int2(cj, __float_as_int(d2));
+                        }
+                        if (lane == qi) my_cnt += __popc(m);
+                    }
+                }
+            });
+            if (has) a.cnt[my_row] = my_cnt;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S8-S10: emit.  Thread per row in ORIGINAL order: capped degrees -> exclusive scan over the whole
+// call (single pass, decoupled look-back: one 64-bit descriptor per tile, [63:62] flag 0 = not
+// ready / 1 = tile aggregate / 2 = inclusive prefix; tiles take their index from an atomic ticket
+// so a tile only waits on tiles that already run) -> CSR row_ptr.  Then every row places its hits
+// at row_ptr[i] + (rank of dst among the row's hits): no sort, the COO comes out (src,dst)-sorted.
+// Rows whose hits did not fit the slot buffer, or with more than k_max hits, are recomputed by the
+// whole warp: exact K-smallest by (d2, j) through bisection on the bit pattern of d2 and then on j
+// among ties (storage-free), hits written unsorted and ordered by a bitonic network in place.
+// ------------------------------------------------------------------------------------------------
+constexpr int kEmitThreads = 512;
+constexpr uint64_t kFlagA = 1ull << 62, kFlagP = 2ull << 62, kValMask = (1ull << 62) - 1;
+
+__device__ __forceinline__ uint64_t ld_relaxed_u64(const uint64_t* p) {
+    uint64_t v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u64(uint64_t* p, uint64_t v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+__device__ __forceinline__ void cmp_swap(int32_t* dst, float* d2, int64_t lo, int64_t hi) {
+    const int32_t x = dst[lo], y = dst[hi];
+    if (x > y) {
+        dst[lo] = y; dst[hi] = x;
+        const float t = d2[lo]; d2[lo] = d2[hi]; d2[hi] = t;
+    }
+}
+
+// in-place ascending sort of (dst, d2)[0..len) by dst, whole warp, any len: bitonic network whose
+// comparators all point upwards, so virtual +inf padding above the row never moves
+__device__ __forceinline__ void warp_sort_rows(int32_t* dst, float* d2, int64_t len, int lane) {
+    int64_t p2 = 1;
+    while (p2 < len) p2 <<= 1;
+    for (int64_t k = 2; k <= p2; k <<= 1) {
+        const int64_t hk = k >> 1;
+        for (int64_t t = lane; t < (p2 >> 1); t += 32) {              // flip stage: i <-> i ^ (k-1)
+            const int64_t lo = (t / hk) * k + (t % hk);
+            const int64_t hi = lo ^ (k - 1);
+            if (hi < len) cmp_swap(dst, d2, lo, hi);
+        }
+        __syncwarp();
+        for (int64_t j = k >> 2; j >= 1; j >>= 1) {
+            for (int64_t t = lane; t < (p2 >> 1); t += 32) {
+                const int64_t lo = (t / j) * (2 * j) + (t % j);
+                const int64_t hi = lo + j;
+                if (hi < len) cmp_swap(dst, d2, lo, hi);
+            }
+            __syncwarp();
+        }
+    }
+}
+
+struct EmitArgs {
+    const float4* pts;            // original points (to recompute the cell of a big row)
+    const float4* spts;
+    const int32_t* sidx;
+    const uint32_t* cell_start;
     const uint32_t* cnt;
-    int64_t* row_ptr;         // [n+1]
+    const int2* hits;
+    const int64_t* ev_off;        // device event offsets (n_events + 1) or NULL for one event
+    int n_events;
+    int64_t n_total;
+    uint64_t* tile_state;
+    uint32_t* ticket;
+    int64_t* row_ptr;             // optional [n_total + 1]
+    int32_t* out_src;
+    int32_t* out_dst;
+    float* out_d2;
+    int64_t capacity;
+    int64_t* out_count;           // optional
+    int64_t* out_edge_offsets;    // optional [n_events + 1]
+    int32_t* out_status;
+    float r2, inv_cell;
+    int bits;
     uint32_t k_max;
-    __device__ __forceinline__ uint64_t value(uint32_t v) const { return v < k_max ? v : k_max; }
-    __device__ __forceinline__ uint32_t load(int64_t i) const { return cnt[i]; }
-    __device__ __forceinline__ void store(int64_t i, uint32_t, uint64_t excl) const { row_ptr[i] = static_cast<int64_t>(excl); }
-    __device__ __forceinline__ void finish(int64_t n, uint64_t total) const { row_ptr[n] = static_cast<int64_t>(total); }
 };
 
-template <class Policy>
-__global__ void __launch_bounds__(kScanThreads) scan_kernel(Policy p, int64_t n, uint64_t* tile_state, uint32_t* ticket) {
-    __shared__ uint64_t s_warp[kScanThreads / 32];
+template <int G>
+__global__ void __launch_bounds__(kEmitThreads) emit_kernel(EmitArgs a) {
+    __shared__ uint64_t s_warp[kEmitThreads / 32];
     __shared__ uint64_t s_prefix;
     __shared__ uint32_t s_tile;
+    __shared__ int s_delta[kEmitThreads / 32][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    if (threadIdx.x == 0) s_tile = atomicAdd(a.ticket, 1u);
     __syncthreads();
     const uint32_t tile = s_tile;
-    const int64_t base = static_cast<int64_t>(tile) * kScanTile + static_cast<int64_t>(threadIdx.x) * kScanItems;
-    uint32_t v[kScanItems];
-    uint64_t tsum = 0;
-#pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        v[k] = (base + k < n) ? p.load(base + k) : 0u;
-        tsum += p.value(v[k]);
-    }
-    uint64_t incl = tsum;
+    const int64_t i = static_cast<int64_t>(tile) * kEmitThreads + threadIdx.x;
+    const bool has = i < a.n_total;
+    const uint32_t c = has ? a.cnt[i] : 0u;
+    const uint32_t deg = c < a.k_max ? c : a.k_max;
+    // ---- block scan of deg
+    uint64_t incl = deg;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        uint64_t t = __shfl_up_sync(kFull, incl, o);
+        const uint64_t t = __shfl_up_sync(kFull, incl, o);
         if (lane >= o) incl += t;
     }
     if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
     uint64_t wexcl = 0, btotal = 0;
 #pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) {
-        uint64_t t = s_warp[w];
+    for (int w = 0; w < kEmitThreads / 32; ++w) {
+        const uint64_t t = s_warp[w];
         if (w < warp) wexcl += t;
         btotal += t;
     }
+    // ---- decoupled look-back for the tile's global offset
     if (warp == 0) {
         uint64_t excl = 0;
-        if (lane == 0) st_volatile_u64(&tile_state[tile], (tile == 0 ? kFlagP : kFlagA) | btotal);
+        if (lane == 0) st_relaxed_u64(&a.tile_state[tile], (tile == 0 ? kFlagP : kFlagA) | btotal);
         if (tile > 0) {
             int look = static_cast<int>(tile) - 1;
             while (true) {
                 const int t = look - lane;
                 uint64_t st = kFlagP;                                  // virtual tile -1: prefix 0
                 if (t >= 0) {
-                    do { st = ld_volatile_u64(&tile_state[t]); } while ((st >> 62) == 0);
+                    do { st = ld_relaxed_u64(&a.tile_state[t]); } while ((st >> 62) == 0);
                 }
                 const uint32_t pmask = __ballot_sync(kFull, (st >> 62) == 2);
                 const int first_p = pmask ? (__ffs(pmask) - 1) : 31;
@@ -217,320 +525,127 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(Policy p, int64_t n,
                 if (pmask) break;
                 look -= 32;
             }
-            if (lane == 0) st_volatile_u64(&tile_state[tile], kFlagP | (excl + btotal));
+            if (lane == 0) st_relaxed_u64(&a.tile_state[tile], kFlagP | (excl + btotal));
         }
         if (lane == 0) s_prefix = excl;
     }
     __syncthreads();
-    uint64_t run = s_prefix + wexcl + (incl - tsum);
-#pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        if (base + k < n) {
-            p.store(base + k, v[k], run);
-            run += p.value(v[k]);
-            if (base + k == n - 1) p.finish(n, run);
+    const int64_t rp = static_cast<int64_t>(s_prefix + wexcl + (incl - deg));      // row_ptr[i]
+    // ---- CSR offsets, count, status, per-event edge offsets
+    int64_t ev_base = 0;
+    if (has) {
+        if (a.row_ptr) a.row_ptr[i] = rp;
+        if (a.ev_off) {
+            int e = event_of_row(a.ev_off, a.n_events, i);
+            ev_base = a.ev_off[e];
+            if (a.out_edge_offsets)
+                for (; e >= 0 && a.ev_off[e] == i; --e) a.out_edge_offsets[e] = rp;    // event starts (and empty events) at row i
+        }
+        if (i == a.n_total - 1) {
+            const int64_t total = rp + deg;
+            if (a.row_ptr) a.row_ptr[a.n_total] = total;
+            if (a.out_count) *a.out_count = total;
+            if (a.out_edge_offsets)
+                for (int e = a.n_events; e >= 0 && a.ev_off[e] == a.n_total; --e) a.out_edge_offsets[e] = total;
+            *a.out_status = total > a.capacity ? -3 /* FRNN_ERR_CAPACITY */ : 0;
         }
     }
-}
-
-// ------------------------------------------------------------------------------------------------
-// S5: neighbour-cell enumeration for one occupied cell.  The last binned coordinate is the
-// fastest-varying one in the linear cell id, so its three adjacent cells are ONE contiguous run of
-// the cell-ordered copy: 3^G cells = 3^(G-1) runs.  Up to 27 runs live in lanes (one per lane);
-// G > 4 loops over 3^(G-4) run groups.  Runs of a group are flattened: an inclusive warp scan of
-// the run lengths, then each lane finds "its" candidate of the current 32-chunk by a 5-step
-// shuffle search.  f(valid, slot) is called once per chunk with one candidate slot per lane.
-// A cell on the 0 / 2^bits-1 face of the last coordinate has its wrapped neighbour in a second
-// pass ("piece 1").
-// ------------------------------------------------------------------------------------------------
-__host__ __device__ constexpr int pow3(int e) { return e <= 0 ? 1 : 3 * pow3(e - 1); }
-
-template <int G, class F>
-__device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, int bits, const uint32_t* __restrict__ cell_start,
-                                                         int lane, F&& f) {
-    constexpr int LD = (G - 1 < 3) ? (G - 1) : 3;     // coordinates enumerated across lanes
-    constexpr int RL = pow3(LD);                      // runs per group (<= 27)
-    constexpr int GD = G - 1 - LD;                    // coordinates enumerated by the group loop
-    constexpr int NG = pow3(GD);
-    const uint32_t mask = (1u << bits) - 1u;
-    const uint32_t c_last = cell & mask;
-    const bool edge_lo = c_last == 0u, edge_hi = c_last == mask;
-    const int n_pieces = (edge_lo || edge_hi) ? 2 : 1;
-    const uint32_t ev = cell >> (G * bits);
-    for (int grp = 0; grp < NG; ++grp) {
-        uint32_t base = ev;
-        {
-            int kk = lane, gg = grp;
-#pragma unroll
-            for (int d = 0; d < G - 1; ++d) {
-                int o;
-                if (d < GD) { o = gg % 3 - 1; gg /= 3; } else { o = kk % 3 - 1; kk /= 3; }
-                const uint32_t cd = (cell >> ((G - 1 - d) * bits)) & mask;
-                base = (base << bits) | ((cd + static_cast<uint32_t>(o)) & mask);
+    // ---- rows that fit their slot buffer: rank by dst, place directly
+    const bool big = has && (c > kSlot || c > a.k_max);
+    if (has && !big && c > 0) {
+        const int2* h = a.hits + i * kSlot;
+        const int32_t src = static_cast<int32_t>(i - ev_base);
+        for (uint32_t m = 0; m < c; ++m) {
+            const int2 mine = h[m];
+            uint32_t rank = 0;
+            for (uint32_t u = 0; u < c; ++u) rank += h[u].x < mine.x;
+            const int64_t pos = rp + rank;
+            if (pos < a.capacity) {
+                a.out_src[pos] = src;
+                a.out_dst[pos] = mine.x - static_cast<int32_t>(ev_base);
+                a.out_d2[pos] = __int_as_float(mine.y);
             }
-            base <<= bits;
         }
-        for (int piece = 0; piece < n_pieces; ++piece) {
-            uint32_t lo, hi;
-            if (piece == 0) { lo = edge_lo ? 0u : c_last - 1u; hi = edge_hi ? mask : c_last + 1u; }
-            else            { lo = hi = edge_lo ? mask : 0u; }
-            uint32_t s = 0, e = 0;
-            if (lane < RL) { s = cell_start[base + lo]; e = cell_start[base + hi + 1u]; }
-            const int len = static_cast<int>(e - s);
-            int incl = len;
+    }
+    // ---- big rows: recompute with the whole warp
+    uint32_t bigs = __ballot_sync(kFull, big);
+    if (bigs == 0) return;
+    const int lane_delta = lane_row_delta<G>(lane, a.bits);
+    const uint32_t mask = (1u << a.bits) - 1u;
+    for (; bigs; bigs &= bigs - 1) {
+        const int bl = __ffs(bigs) - 1;
+        const int64_t row = __shfl_sync(kFull, i, bl);
+        const int64_t row_rp = __shfl_sync(kFull, rp, bl);
+        const int64_t row_ev = __shfl_sync(kFull, ev_base, bl);
+        const uint32_t row_cnt = __shfl_sync(kFull, c, bl);
+        const float4 qa = a.pts[2 * row], qb = a.pts[2 * row + 1];
+        uint32_t ev = 0;
+        if (a.ev_off) ev = static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, row));
+        const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, a.bits);
+        bool interior = true;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int t = __shfl_up_sync(kFull, incl, o);
-                if (lane >= o) incl += t;
-            }
-            const int total = __shfl_sync(kFull, incl, 31);
-            const int delta = static_cast<int>(s) - (incl - len);     // slot = t + delta for t in this run
-            for (int b = 0; b < total; b += 32) {
-                const int t = b + lane;
-                int k = 0;
-#pragma unroll
-                for (int step = 16; step >= 1; step >>= 1) {
-                    const int pk = __shfl_sync(kFull, incl, (k + step - 1) & 31);
-                    if (pk <= t) k += step;
+        for (int d = 0; d < G; ++d) {
+            const uint32_t cd = (cell >> (d * a.bits)) & mask;
+            interior = interior && cd != 0u && cd != mask;
+        }
+        const float inf = __int_as_float(0x7f800000);
+        // visit(g): g(hit_candidate_lane, j, d2) once per chunk with the in-radius test applied
+        auto visit = [&](auto&& g) {
+            for_each_candidate_chunk<G>(cell, interior, a.bits, lane_delta, a.cell_start, s_delta[warp], lane, [&](int cslot) {
+                float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
+                int32_t cj = -1;
+                if (cslot >= 0) {
+                    ca = a.spts[2 * static_cast<int64_t>(cslot)];
+                    cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
+                    cj = a.sidx[cslot];
                 }
-                const int slot = t + __shfl_sync(kFull, delta, k & 31);
-                f(t < total, slot);
-            }
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// S6..S8, S10: search.  One warp per segment (occupied cell), persistent grid-stride over the
-// segment list.  Queries = the cell's points (<= 32 per pass), staged once in shared memory and
-// read back as broadcasts; candidates = one per lane per chunk.  PASS 0 counts |S_i| (uncapped);
-// PASS 1 writes the kept hits of every row with |S_i| <= k_max unsorted at row_ptr[i] (the row is
-// ordered by dst in sort_rows_kernel) and resolves overflowing rows with a storage-free exact
-// selection: bisection on the bit pattern of d2, then on j among ties (S8).
-// ------------------------------------------------------------------------------------------------
-constexpr int kSearchWarps = 8;
-
-struct SearchArgs {
-    const float4* spts;
-    const int32_t* sidx;          // slot -> global row index
-    const uint32_t* cell_start;
-    const Segment* segs;
-    const uint32_t* n_segs;
-    const int64_t* ev_off;        // device copy of the event offsets (n_events + 1); NULL = one event
-    uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index
-    const int64_t* row_ptr;
-    int32_t* out_src;
-    int32_t* out_dst;
-    float* out_d2;
-    int64_t capacity;
-    float r2;
-    int bits;
-    uint32_t k_max;
-};
-
-template <int G, int PASS>
-__global__ void __launch_bounds__(kSearchWarps * 32) search_kernel(SearchArgs a) {
-    __shared__ float4 s_q[kSearchWarps][64];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-    const uint32_t n_segs = *a.n_segs;
-    const uint32_t stride = gridDim.x * kSearchWarps;
-    float4* q = s_q[warp];
-    for (uint32_t sg = blockIdx.x * kSearchWarps + warp; sg < n_segs; sg += stride) {
-        const Segment seg = a.segs[sg];
-        const int64_t ev_base = a.ev_off ? a.ev_off[seg.cell >> (G * a.bits)] : 0;
-        for (uint32_t q0 = 0; q0 < seg.len; q0 += 32) {
-            const int nq = min(32u, seg.len - q0);
-            const uint32_t my_slot = seg.start + q0 + lane;
-            const bool has = lane < nq;
-            int32_t my_row = -1;
-            __syncwarp();
-            if (has) {
-                q[2 * lane] = a.spts[2 * static_cast<int64_t>(my_slot)];
-                q[2 * lane + 1] = a.spts[2 * static_cast<int64_t>(my_slot) + 1];
-                my_row = a.sidx[my_slot];
-            }
-            __syncwarp();
-            if (PASS == 0) {
-                uint32_t my_cnt = 0;
-                for_each_candidate_chunk<G>(seg.cell, a.bits, a.cell_start, lane, [&](bool valid, int cslot) {
-                    float4 ca = make_float4(0.f, 0.f, 0.f, 0.f), cb = ca;
-                    if (valid) { ca = a.spts[2 * static_cast<int64_t>(cslot)]; cb = a.spts[2 * static_cast<int64_t>(cslot) + 1]; }
-                    for (int qi = 0; qi < nq; ++qi) {
-                        const float d2 = d2_pinned(q[2 * qi], q[2 * qi + 1], ca, cb);
-                        const bool hit = valid && d2 <= a.r2 && static_cast<uint32_t>(cslot) != seg.start + q0 + qi;
-                        const uint32_t m = __ballot_sync(kFull, hit);
-                        if (lane == qi) my_cnt += __popc(m);
-                    }
+                const float d2 = d2_pinned(qa, qb, ca, cb);
+                g(d2 <= a.r2 && cj != static_cast<int32_t>(row), cj, d2);
+            });
+        };
+        // threshold key (dthr, jthr): keep hits with (d2 bits, j) <= it.  d2 >= +0 always (the chain
+        // starts at +0 and adds squares), so bit patterns order like values.
+        uint32_t dthr = __float_as_uint(a.r2);
+        int32_t jthr = 0x7fffffff;
+        if (row_cnt > a.k_max) {
+            auto count_le = [&](uint32_t dkey, int32_t jkey) -> uint32_t {
+                uint32_t n = 0;
+                visit([&](bool in, int32_t cj, float d2) {
+                    const uint32_t db = __float_as_uint(d2);
+                    n += __popc(__ballot_sync(kFull, in && (db < dkey || (db == dkey && cj <= jkey))));
                 });
-                if (has) a.cnt[my_row] = my_cnt;
-            } else {
-                const uint32_t my_cnt = has ? a.cnt[my_row] : 0u;
-                const int64_t my_rp = has ? a.row_ptr[my_row] : 0;
-                const int32_t my_src = my_row - static_cast<int32_t>(ev_base);
-                uint32_t my_off = 0;
-                const uint32_t normal = __ballot_sync(kFull, has && my_cnt > 0 && my_cnt <= a.k_max);
-                uint32_t over = __ballot_sync(kFull, has && my_cnt > a.k_max);
-                if (normal) {
-                    for_each_candidate_chunk<G>(seg.cell, a.bits, a.cell_start, lane, [&](bool valid, int cslot) {
-                        float4 ca = make_float4(0.f, 0.f, 0.f, 0.f), cb = ca;
-                        int32_t cj = 0;
-                        if (valid) {
-                            ca = a.spts[2 * static_cast<int64_t>(cslot)]; cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
-                            cj = a.sidx[cslot] - static_cast<int32_t>(ev_base);
-                        }
-                        for (uint32_t rem = normal; rem; rem &= rem - 1) {
-                            const int qi = __ffs(rem) - 1;
-                            const float d2 = d2_pinned(q[2 * qi], q[2 * qi + 1], ca, cb);
-                            const bool hit = valid && d2 <= a.r2 && static_cast<uint32_t>(cslot) != seg.start + q0 + qi;
-                            const uint32_t m = __ballot_sync(kFull, hit);
-                            if (m) {
-                                const int64_t rp = __shfl_sync(kFull, my_rp, qi);
-                                const uint32_t off = __shfl_sync(kFull, my_off, qi);
-                                const int32_t src = __shfl_sync(kFull, my_src, qi);
-                                if (hit) {
-                                    const int64_t pos = rp + off + __popc(m & lt_mask);
-                                    if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = cj; a.out_d2[pos] = d2; }
-                                }
-                                if (lane == qi) my_off += __popc(m);
-                            }
-                        }
-                    });
-                }
-                // S8: rows with more than k_max in-radius neighbours.  Exact K-smallest by (d2, j)
-                // without storage: find the threshold key by bisection (every probe re-scans the
-                // candidates), then emit the rows' hits with key <= threshold.
-                for (; over; over &= over - 1) {
-                    const int qi = __ffs(over) - 1;
-                    const float4 qa = q[2 * qi], qb = q[2 * qi + 1];
-                    const uint32_t self_slot = seg.start + q0 + qi;
-                    auto count_le = [&](uint32_t dkey, int32_t jkey) -> uint32_t {   // #{(d2,j) <= (dkey,jkey)}
-                        uint32_t c = 0;
-                        for_each_candidate_chunk<G>(seg.cell, a.bits, a.cell_start, lane, [&](bool valid, int cslot) {
-                            float4 ca = make_float4(0.f, 0.f, 0.f, 0.f), cb = ca;
-                            int32_t cj = 0;
-                            if (valid) {
-                                ca = a.spts[2 * static_cast<int64_t>(cslot)]; cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
-                                cj = a.sidx[cslot];
-                            }
-                            const float d2 = d2_pinned(qa, qb, ca, cb);
-                            const uint32_t db = __float_as_uint(d2);
-                            const bool hit = valid && d2 <= a.r2 && static_cast<uint32_t>(cslot) != self_slot &&
-                                             (db < dkey || (db == dkey && cj <= jkey));
-                            c += __popc(__ballot_sync(kFull, hit));
-                        });
-                        return c;
-                    };
-                    // d2 >= +0 always (acc starts at +0 and only adds squares): bit patterns order like values
-                    uint32_t dlo = 0, dhi = __float_as_uint(a.r2);
-                    while (dlo < dhi) {
-                        const uint32_t mid = dlo + ((dhi - dlo) >> 1);
-                        if (count_le(mid, 0x7fffffff) >= a.k_max) dhi = mid; else dlo = mid + 1;
-                    }
-                    int32_t jlo = 0, jhi = 0x7fffffff;
-                    while (jlo < jhi) {
-                        const int32_t mid = jlo + ((jhi - jlo) >> 1);
-                        if (count_le(dlo, mid) >= a.k_max) jhi = mid; else jlo = mid + 1;
-                    }
-                    const uint32_t dthr = dlo;
-                    const int32_t jthr = jlo;
-                    const int64_t rp = __shfl_sync(kFull, my_rp, qi);
-                    const int32_t src = __shfl_sync(kFull, my_src, qi);
-                    uint32_t off = 0;
-                    for_each_candidate_chunk<G>(seg.cell, a.bits, a.cell_start, lane, [&](bool valid, int cslot) {
-                        float4 ca = make_float4(0.f, 0.f, 0.f, 0.f), cb = ca;
-                        int32_t cj = 0;
-                        if (valid) {
-                            ca = a.spts[2 * static_cast<int64_t>(cslot)]; cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
-                            cj = a.sidx[cslot];
-                        }
-                        const float d2 = d2_pinned(qa, qb, ca, cb);
-                        const uint32_t db = __float_as_uint(d2);
-                        const bool hit = valid && d2 <= a.r2 && static_cast<uint32_t>(cslot) != self_slot &&
-                                         (db < dthr || (db == dthr && cj <= jthr));
-                        const uint32_t m = __ballot_sync(kFull, hit);
-                        if (hit) {
-                            const int64_t pos = rp + off + __popc(m & lt_mask);
-                            if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = cj - static_cast<int32_t>(ev_base); a.out_d2[pos] = d2; }
-                        }
-                        off += __popc(m);
-                    });
-                }
+                return n;
+            };
+            uint32_t dlo = 0, dhi = dthr;
+            while (dlo < dhi) {
+                const uint32_t mid = dlo + ((dhi - dlo) >> 1);
+                if (count_le(mid, 0x7fffffff) >= a.k_max) dhi = mid; else dlo = mid + 1;
             }
-        }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// S10 (ordering) + call epilogue.  Thread per row: insertion sort of short rows directly in the
-// output arrays; longer rows are sorted by the whole warp with a bitonic network whose comparators
-// all point upwards, so virtual +inf padding above the row never moves (any row length works).
-// Block 0 also publishes count / status / per-event edge offsets.
-// ------------------------------------------------------------------------------------------------
-constexpr int kSmallRow = 12;
-
-__device__ __forceinline__ void cmp_swap(int32_t* dst, float* d2, int64_t lo, int64_t hi) {
-    const int32_t a = dst[lo], b = dst[hi];
-    if (a > b) {
-        dst[lo] = b; dst[hi] = a;
-        const float x = d2[lo]; d2[lo] = d2[hi]; d2[hi] = x;
-    }
-}
-
-__global__ void __launch_bounds__(256) sort_rows_kernel(const int64_t* row_ptr, int64_t n_total, int64_t capacity,
-                                                        int32_t* dst, float* d2,
-                                                        const int64_t* ev_off, int n_events,
-                                                        int64_t* out_count, int64_t* out_edge_offsets, int32_t* out_status) {
-    const int lane = threadIdx.x & 31;
-    const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (blockIdx.x == 0) {
-        const int64_t total = row_ptr[n_total];
-        if (threadIdx.x == 0) {
-            if (out_count) *out_count = total;
-            *out_status = total > capacity ? -3 /* FRNN_ERR_CAPACITY */ : 0;
-        }
-        if (out_edge_offsets)
-            for (int e = threadIdx.x; e <= n_events; e += blockDim.x) out_edge_offsets[e] = row_ptr[ev_off[e]];
-    }
-    int64_t b = 0, len = 0;
-    if (i < n_total) {
-        b = row_ptr[i];
-        const int64_t e = row_ptr[i + 1];
-        len = e <= capacity ? e - b : 0;          // rows cut by the capacity are left as they are
-    }
-    if (len >= 2 && len <= kSmallRow) {
-        for (int64_t u = b + 1; u < b + len; ++u) {
-            const int32_t kj = dst[u];
-            const float kd = d2[u];
-            int64_t v = u - 1;
-            while (v >= b && dst[v] > kj) { dst[v + 1] = dst[v]; d2[v + 1] = d2[v]; --v; }
-            dst[v + 1] = kj; d2[v + 1] = kd;
-        }
-    }
-    uint32_t big = __ballot_sync(kFull, len > kSmallRow);
-    for (; big; big &= big - 1) {
-        const int src_lane = __ffs(big) - 1;
-        const int64_t rb = __shfl_sync(kFull, b, src_lane);
-        const int64_t rl = __shfl_sync(kFull, len, src_lane);
-        int64_t p2 = 1;
-        while (p2 < rl) p2 <<= 1;
-        for (int64_t k = 2; k <= p2; k <<= 1) {
-            const int64_t hk = k >> 1;
-            for (int64_t t = lane; t < (p2 >> 1); t += 32) {          // flip stage: i <-> i ^ (k-1)
-                const int64_t lo = (t / hk) * k + (t % hk);
-                const int64_t hi = lo ^ (k - 1);
-                if (hi < rl) cmp_swap(dst + rb, d2 + rb, lo, hi);
+            int32_t jlo = 0, jhi = 0x7fffffff;
+            while (jlo < jhi) {
+                const int32_t mid = jlo + ((jhi - jlo) >> 1);
+                if (count_le(dlo, mid) >= a.k_max) jhi = mid; else jlo = mid + 1;
             }
-            __syncwarp();
-            for (int64_t j = k >> 2; j >= 1; j >>= 1) {
-                for (int64_t t = lane; t < (p2 >> 1); t += 32) {
-                    const int64_t lo = (t / j) * (2 * j) + (t % j);
-                    const int64_t hi = lo + j;
-                    if (hi < rl) cmp_swap(dst + rb, d2 + rb, lo, hi);
-                }
-                __syncwarp();
-            }
+            dthr = dlo;
+            jthr = jlo;
         }
+        const int32_t src = static_cast<int32_t>(row - row_ev);
+        uint32_t off = 0;
+        visit([&](bool in, int32_t cj, float d2) {
+            const uint32_t db = __float_as_uint(d2);
+            const bool keep = in && (db < dthr || (db == dthr && cj <= jthr));
+            const uint32_t m = __ballot_sync(kFull, keep);
+            if (keep) {
+                const int64_t pos = row_rp + off + __popc(m & lt_mask);
+                if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = cj - static_cast<int32_t>(row_ev); a.out_d2[pos] = d2; }
+            }
+            off += __popc(m);
+        });
+        __syncwarp();
+        const int64_t kept = row_cnt < a.k_max ? row_cnt : a.k_max;
+        if (row_rp + kept <= a.capacity)                       // rows cut by the capacity stay unsorted
+            warp_sort_rows(a.out_dst + row_rp, a.out_d2 + row_rp, kept, lane);
+        __syncwarp();
     }
 }
 

@@ -41,6 +41,7 @@ _SIGNATURES = {
     "frnn_build_host": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
                                    _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64, _c.POINTER(_c.c_int64)]),
     "frnn_last_launch_count": (_c.c_int, []),
+    "frnn_set_graph_mode": (_c.c_int, [_c.c_int]),
     "frnn_set_profiling": (_c.c_int, [_c.c_int]),
     "frnn_get_profile": (_c.c_int, [_c.POINTER(_c.c_float), _c.c_int]),
     "frnn_phase_name": (_c.c_char_p, [_c.c_int]),
@@ -101,6 +102,10 @@ def frnn_get_grid(n_total: int, n_events: int = 1) -> tuple[int, int]:
     d, b = _c.c_int(0), _c.c_int(0)
     lib().frnn_get_grid(int(n_total), int(n_events), _c.byref(d), _c.byref(b))
     return d.value, b.value
+
+
+def frnn_set_graph_mode(enabled: bool) -> None:
+    _check(lib().frnn_set_graph_mode(int(bool(enabled))), "frnn_set_graph_mode")
 
 
 def frnn_last_launch_count() -> int:
