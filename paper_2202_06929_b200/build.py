@@ -20,7 +20,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     tmp = LIB + f".{os.getpid()}.tmp"
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    res = subprocess.run([nvcc, *NVCC_FLAGS, *SOURCES, "-o", tmp], capture_output=True, text=True)
+    extra = os.environ.get("FRNN_NVCC_EXTRA", "").split()          # e.g. -DFRNN_SEARCH_MIN_BLOCKS=4 for sweeps
+    res = subprocess.run([nvcc, *NVCC_FLAGS, *extra, *SOURCES, "-o", tmp], capture_output=True, text=True)
     if verbose or res.returncode != 0:
         print(res.stdout)
         print(res.stderr)

@@ -69,11 +69,12 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     const int64_t row_len = (1ll << g.bits) + 1;
     const int64_t n_rows = L.n_cells >> g.bits;
     L.n_entries = n_rows * row_len;
-    L.rows_per_block = static_cast<int>(4096 / row_len > 0 ? 4096 / row_len : 1);
+    L.rows_per_block = static_cast<int>((kCellTile / row_len) & ~3ll);      // multiple of 4: every block starts 16-byte aligned
+    if (L.rows_per_block < 4) L.rows_per_block = 4;
     L.scan_blocks = (n_rows + L.rows_per_block - 1) / L.rows_per_block;
     L.emit_tiles = (n_total + kEmitThreads - 1) / kEmitThreads;
     size_t o = 0;
-    L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_entries + 1) * 4);
+    L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_entries + 8) * 4);
     L.off_tiles = o;    o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8);
     L.off_counters = o; o = align_up(o + 64);          // [0..7] cursor (u64), [8..11] emit ticket
     L.zero_bytes = o;
@@ -170,9 +171,8 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     const int64_t n_total = c.ev_off[c.n_events];
     char* ws = static_cast<char*>(c.workspace);
     uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
-    uint64_t* tiles = reinterpret_cast<uint64_t*>(ws + L.off_tiles);
+    unsigned long long* tile_deg = reinterpret_cast<unsigned long long*>(ws + L.off_tiles);
     unsigned long long* cursor = reinterpret_cast<unsigned long long*>(ws + L.off_counters);
-    uint32_t* ticket = reinterpret_cast<uint32_t*>(ws + L.off_counters + 8);
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
@@ -219,14 +219,14 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
 
     SearchArgs sa;
     sa.spts = spts; sa.sidx = sidx; sa.cell_start = cells; sa.segs = segs; sa.cursor = cursor; sa.cnt = cnt; sa.hits = hits;
-    sa.r2 = r2; sa.bits = bits;
+    sa.tile_deg = tile_deg; sa.r2 = r2; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
     const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
     FRNN_DISPATCH_G(G, CK((launch_search<GG>(sa, max_segs, st))));
     mark(4, st);
 
     EmitArgs ea;
     ea.pts = pts; ea.spts = spts; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
-    ea.n_events = c.n_events; ea.n_total = n_total; ea.tile_state = tiles; ea.ticket = ticket; ea.row_ptr = c.out_row_ptr;
+    ea.tile_deg = tile_deg; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
     ea.k_max = static_cast<uint32_t>(c.k_max);

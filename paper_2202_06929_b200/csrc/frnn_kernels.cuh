@@ -141,77 +141,79 @@ struct Segment {          // one occupied cell: the unit of work of the search k
 };
 
 constexpr int kCellThreads = 1024;
+constexpr int kCellTile = 4 * kCellThreads;      // table entries per block (upper bound)
 
-// A block owns `rows_per_block` whole padded rows, i.e. rows_per_block * (2^bits + 1) entries.
+// A block owns `rows_per_block` whole padded rows = rows_per_block * (2^bits + 1) <= kCellTile
+// entries (a multiple of 4, so every thread moves one aligned uint4).
 template <int G>
 __global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __restrict__ cells, int64_t n_entries, int rows_per_block,
                                                                  int bits, Segment* __restrict__ segs,
                                                                  unsigned long long* __restrict__ cursor) {
-    __shared__ uint64_t s_warp[kCellThreads / 32];
-    __shared__ uint64_t s_base;
+    __shared__ uint32_t s_pts[32], s_occ[32];
+    __shared__ unsigned long long s_base;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int row_len = (1 << bits) + 1;
-    const int64_t blk_entries = static_cast<int64_t>(rows_per_block) * row_len;
+    const uint32_t row_len = (1u << bits) + 1u;
+    const uint32_t blk_entries = static_cast<uint32_t>(rows_per_block) * row_len;
     const int64_t blk_base = static_cast<int64_t>(blockIdx.x) * blk_entries;
-    const int64_t blk_end = min(blk_base + blk_entries, n_entries);
-    const uint32_t mask = (1u << bits) - 1u;
-    uint64_t carry = 0;                                   // (occupied << 32 | points) of earlier strips
-    // pass 1: block total (so that ONE atomic reserves the block's range), strip by strip
-    uint64_t tsum = 0;
-    for (int64_t i = blk_base + threadIdx.x; i < blk_end; i += kCellThreads) {
-        const uint32_t v = cells[i];
-        tsum += (static_cast<uint64_t>(v != 0) << 32) | v;
-    }
+    const uint32_t local = threadIdx.x * 4u;
+    const bool act = local < blk_entries && blk_base + local < n_entries;      // n_entries is a multiple of 4 as well
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (act) v = *reinterpret_cast<const uint4*>(cells + blk_base + local);
+    const uint32_t tp = v.x + v.y + v.z + v.w;
+    const uint32_t to = (v.x != 0u) + (v.y != 0u) + (v.z != 0u) + (v.w != 0u);
+    uint32_t ip = tp, io = to;                                                 // inclusive warp scans
 #pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) tsum += __shfl_xor_sync(kFull, tsum, o);
-    if (lane == 0) s_warp[warp] = tsum;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint64_t t = 0;
-        for (int w = 0; w < kCellThreads / 32; ++w) t += s_warp[w];
-        s_base = t ? atomicAdd(cursor, static_cast<unsigned long long>(t)) : 0ull;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t a = __shfl_up_sync(kFull, ip, o), b = __shfl_up_sync(kFull, io, o);
+        if (lane >= o) { ip += a; io += b; }
     }
+    if (lane == 31) { s_pts[warp] = ip; s_occ[warp] = io; }
     __syncthreads();
-    carry = s_base;
-    __syncthreads();
-    // pass 2: exclusive scan strip by strip (the strip's counts are L1/L2 hits now)
-    for (int64_t s0 = blk_base; s0 < blk_end; s0 += kCellThreads) {
-        const int64_t i = s0 + threadIdx.x;
-        const uint32_t v = i < blk_end ? cells[i] : 0u;
-        const uint64_t val = (static_cast<uint64_t>(v != 0) << 32) | v;
-        uint64_t incl = val;
+    if (warp == 0) {
+        const uint32_t wp = s_pts[lane], wo = s_occ[lane];
+        uint32_t sp = wp, so = wo;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const uint64_t t = __shfl_up_sync(kFull, incl, o);
-            if (lane >= o) incl += t;
+            const uint32_t a = __shfl_up_sync(kFull, sp, o), b = __shfl_up_sync(kFull, so, o);
+            if (lane >= o) { sp += a; so += b; }
         }
-        if (lane == 31) s_warp[warp] = incl;
-        __syncthreads();
-        uint64_t wexcl = 0, total = 0;
+        s_pts[lane] = sp - wp;                                                 // exclusive warp offsets
+        s_occ[lane] = so - wo;
+        if (lane == 31) {
+            const unsigned long long total = (static_cast<unsigned long long>(so) << 32) | sp;
+            s_base = total ? atomicAdd(cursor, total) : 0ull;
+        }
+    }
+    __syncthreads();
+    if (!act) return;
+    const unsigned long long base = s_base;
+    uint32_t p = static_cast<uint32_t>(base) + s_pts[warp] + (ip - tp);
+    uint32_t oc = static_cast<uint32_t>(base >> 32) + s_occ[warp] + (io - to);
+    const uint32_t cnt[4] = {v.x, v.y, v.z, v.w};
+    uint4 out;
+    out.x = p; out.y = p + v.x; out.z = out.y + v.y; out.w = out.z + v.z;
+    *reinterpret_cast<uint4*>(cells + blk_base + local) = out;
+    if (to) {
+        const uint32_t mask = (1u << bits) - 1u;
+        const float inv_row = 1.0f / static_cast<float>(row_len);
 #pragma unroll
-        for (int w = 0; w < kCellThreads / 32; ++w) {
-            const uint64_t t = s_warp[w];
-            if (w < warp) wexcl += t;
-            total += t;
-        }
-        const uint64_t excl = carry + wexcl + (incl - val);
-        if (i < blk_end) {
-            cells[i] = static_cast<uint32_t>(excl);
-            if (v) {
-                // table index -> linear id: remove the padding entries (row = i / row_len)
-                const uint32_t row = static_cast<uint32_t>(i / row_len);
-                const uint32_t lin = static_cast<uint32_t>(i) - row;
+        for (int k = 0; k < 4; ++k) {
+            if (cnt[k]) {
+                // table index -> linear id: drop the padding entries of the rows before this one
+                const uint32_t e = local + k;
+                const uint32_t row_local = __float2uint_rz((static_cast<float>(e) + 0.5f) * inv_row);     // e / row_len, e < 4096
+                const uint32_t lin = static_cast<uint32_t>(blk_base + e) - (blockIdx.x * static_cast<uint32_t>(rows_per_block) + row_local);
                 bool interior = true;
 #pragma unroll
                 for (int d = 0; d < G; ++d) {
                     const uint32_t c = (lin >> (d * bits)) & mask;
                     interior = interior && c != 0u && c != mask;
                 }
-                segs[excl >> 32] = Segment{lin, static_cast<uint32_t>(excl), v, interior ? 1u : 0u};
+                segs[oc] = Segment{lin, p, cnt[k], interior ? 1u : 0u};
+                ++oc;
             }
+            p += cnt[k];
         }
-        carry += total;
-        __syncthreads();
     }
 }
 
@@ -252,8 +254,8 @@ __device__ __forceinline__ int lane_row_delta(int lane, int bits) {
     return delta;
 }
 
-template <int G, class F>
-__device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, bool interior, int bits, int lane_delta,
+template <int G, bool INTERIOR, class F>
+__device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, int bits, int lane_delta,
                                                          const uint32_t* __restrict__ cell_start, int* s_delta,
                                                          int lane, F&& f) {
     using N = Neigh<G>;
@@ -261,10 +263,10 @@ __device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, bool int
     const uint32_t c_last = cell & mask;
     const uint32_t lt_mask = (1u << lane) - 1u;
     const bool edge_lo = c_last == 0u, edge_hi = c_last == mask;
-    const int n_pieces = (!interior && (edge_lo || edge_hi)) ? 2 : 1;
+    const int n_pieces = (!INTERIOR && (edge_lo || edge_hi)) ? 2 : 1;
     for (int grp = 0; grp < N::NG; ++grp) {
         uint32_t row;                                        // padded table index of the neighbour row's cell 0
-        if (interior) {
+        if (INTERIOR) {
             int gdelta = 0, gg = grp;
 #pragma unroll
             for (int d = 0; d < N::GD; ++d) { gdelta += (gg % 3 - 1) * (1 << ((G - 1 - d) * bits)); gg /= 3; }
@@ -283,8 +285,9 @@ __device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, bool int
         }
         for (int piece = 0; piece < n_pieces; ++piece) {
             uint32_t lo, hi;
-            if (piece == 0) { lo = edge_lo ? 0u : c_last - 1u; hi = edge_hi ? mask : c_last + 1u; }
-            else            { lo = hi = edge_lo ? mask : 0u; }
+            if (INTERIOR)        { lo = c_last - 1u; hi = c_last + 1u; }
+            else if (piece == 0) { lo = edge_lo ? 0u : c_last - 1u; hi = edge_hi ? mask : c_last + 1u; }
+            else                 { lo = hi = edge_lo ? mask : 0u; }
             uint32_t s = 0, e = 0;
             if (lane < N::RL) { s = cell_start[row + lo]; e = cell_start[row + hi + 1u]; }
             const int len = static_cast<int>(e - s);
@@ -324,7 +327,12 @@ __device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, bool int
 // which tells emit_kernel to resolve that row by recomputation.
 // ------------------------------------------------------------------------------------------------
 constexpr int kSearchWarps = 8;
+// ptxas caps registers from the launch bounds: 5 resident blocks of 256 threads = 48 registers.
+#ifndef FRNN_SEARCH_MIN_BLOCKS
+#define FRNN_SEARCH_MIN_BLOCKS 5
+#endif
 constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
+constexpr int kEmitThreads = 512;      // rows per emit tile
 
 struct SearchArgs {
     const float4* spts;
@@ -334,88 +342,96 @@ struct SearchArgs {
     const unsigned long long* cursor;   // high 32 bits = number of segments
     uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index
     int2* hits;                   // [n_total * kSlot] (j global, d2 bits)
+    unsigned long long* tile_deg; // [ceil(n_total / kEmitThreads)] sum of min(|S_i|, k_max) per emit tile (zeroed)
     float r2;
     int bits;
+    uint32_t k_max;
 };
 
+template <int G, bool INTERIOR>
+__device__ __forceinline__ void search_segment(const SearchArgs& a, const Segment& seg, float4* q, int* s_delta, int lane,
+                                               int lane_delta, uint32_t lt_mask) {
+    const float inf = __int_as_float(0x7f800000);
+    for (uint32_t q0 = 0; q0 < seg.len; q0 += 32) {
+        const int nq = min(32u, seg.len - q0);
+        const uint32_t first_slot = seg.start + q0;
+        const bool has = lane < nq;
+        int32_t my_row = 0;
+        uint32_t my_cnt = 0;
+        __syncwarp();
+        if (has) {
+            q[2 * lane] = a.spts[2 * static_cast<int64_t>(first_slot + lane)];
+            q[2 * lane + 1] = a.spts[2 * static_cast<int64_t>(first_slot + lane) + 1];
+            my_row = a.sidx[first_slot + lane];
+        }
+        __syncwarp();
+        for_each_candidate_chunk<G, INTERIOR>(seg.cell, a.bits, lane_delta, a.cell_start, s_delta, lane, [&](int cslot) {
+            float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);   // no candidate: d2 = inf
+            int32_t cj = 0;
+            if (cslot >= 0) {
+                ca = a.spts[2 * static_cast<int64_t>(cslot)];
+                cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
+                cj = a.sidx[cslot];
+            }
+            const int self_q = cslot - static_cast<int>(first_slot);   // the query this candidate IS (if in [0, nq))
+            for (int qi = 0; qi < nq; ++qi) {
+                const float d2 = d2_pinned(q[2 * qi], q[2 * qi + 1], ca, cb);
+                const bool hit = d2 <= a.r2 && self_q != qi;
+                const uint32_t m = __ballot_sync(kFull, hit);
+                if (m) {
+                    const uint32_t base = __shfl_sync(kFull, my_cnt, qi);
+                    const int32_t row = __shfl_sync(kFull, my_row, qi);
+                    if (hit) {
+                        const uint32_t pos = base + __popc(m & lt_mask);
+                        if (pos < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + pos] = make_int2(cj, __float_as_int(d2));
+                    }
+                    if (lane == qi) my_cnt += __popc(m);
+                }
+            }
+        });
+        if (has) {
+            a.cnt[my_row] = my_cnt;
+            // per-tile degree totals: emit_kernel turns them into its global offsets without any
+            // inter-block wait
+            if (my_cnt) atomicAdd(&a.tile_deg[my_row / kEmitThreads], static_cast<unsigned long long>(my_cnt < a.k_max ? my_cnt : a.k_max));
+        }
+    }
+}
+
 template <int G>
-__global__ void __launch_bounds__(kSearchWarps * 32) search_kernel(SearchArgs a) {
+__global__ void __launch_bounds__(kSearchWarps * 32, FRNN_SEARCH_MIN_BLOCKS) search_kernel(SearchArgs a) {
     __shared__ float4 s_q[kSearchWarps][64];
     __shared__ int s_delta[kSearchWarps][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t n_segs = static_cast<uint32_t>(*a.cursor >> 32);
     const uint32_t stride = gridDim.x * kSearchWarps;
-    const int lane_delta = lane_row_delta<G>(lane, a.bits);
-    float4* q = s_q[warp];
-    const float inf = __int_as_float(0x7f800000);
-    for (uint32_t sg = blockIdx.x * kSearchWarps + warp; sg < n_segs; sg += stride) {
-        const Segment seg = a.segs[sg];
-        for (uint32_t q0 = 0; q0 < seg.len; q0 += 32) {
-            const int nq = min(32u, seg.len - q0);
-            const uint32_t first_slot = seg.start + q0;
-            const bool has = lane < nq;
-            int32_t my_row = 0;
-            uint32_t my_cnt = 0;
-            __syncwarp();
-            if (has) {
-                q[2 * lane] = a.spts[2 * static_cast<int64_t>(first_slot + lane)];
-                q[2 * lane + 1] = a.spts[2 * static_cast<int64_t>(first_slot + lane) + 1];
-                my_row = a.sidx[first_slot + lane];
-            }
-            __syncwarp();
-            for_each_candidate_chunk<G>(seg.cell, seg.interior != 0u, a.bits, lane_delta, a.cell_start, s_delta[warp], lane,
-                                        [&](int cslot) {
-                float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);   // no candidate: d2 = inf
-                int32_t cj = 0;
-                if (cslot >= 0) {
-                    ca = a.spts[2 * static_cast<int64_t>(cslot)];
-                    cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
-                    cj = a.sidx[cslot];
-                }
-                const int self_q = cslot - static_cast<int>(first_slot);   // the query this candidate IS (if in [0, nq))
-                for (int qi = 0; qi < nq; ++qi) {
-                    const float d2 = d2_pinned(q[2 * qi], q[2 * qi + 1], ca, cb);
-                    const bool hit = d2 <= a.r2 && self_q != qi;
-                    const uint32_t m = __ballot_sync(kFull, hit);
-                    if (m) {
-                        const uint32_t base = __shfl_sync(kFull, my_cnt, qi);
-                        const int32_t row = __shfl_sync(kFull, my_row, qi);
-                        if (hit) {
-                            const uint32_t pos = base + __popc(m & lt_mask);
-                            if (pos < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + pos] = make_int2(cj, __float_as_int(d2));
-                        }
-                        if (lane == qi) my_cnt += __popc(m);
-                    }
-                }
-            });
-            if (has) a.cnt[my_row] = my_cnt;
-        }
+    int lane_delta = lane_row_delta<G>(lane, a.bits);
+    asm volatile("" : "+r"(lane_delta));                  // keep it in a register: do not recompute per segment
+    uint32_t sg = blockIdx.x * kSearchWarps + warp;
+    if (sg >= n_segs) return;
+    Segment seg = a.segs[sg];
+    while (true) {
+        const uint32_t nxt = sg + stride;
+        Segment seg_next = seg;
+        if (nxt < n_segs) seg_next = a.segs[nxt];         // prefetch: the load overlaps this segment's work
+        if (seg.interior) search_segment<G, true>(a, seg, s_q[warp], s_delta[warp], lane, lane_delta, lt_mask);
+        else              search_segment<G, false>(a, seg, s_q[warp], s_delta[warp], lane, lane_delta, lt_mask);
+        if (nxt >= n_segs) break;
+        sg = nxt;
+        seg = seg_next;
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// S8-S10: emit.  Thread per row in ORIGINAL order: capped degrees -> exclusive scan over the whole
-// call (single pass, decoupled look-back: one 64-bit descriptor per tile, [63:62] flag 0 = not
-// ready / 1 = tile aggregate / 2 = inclusive prefix; tiles take their index from an atomic ticket
-// so a tile only waits on tiles that already run) -> CSR row_ptr.  Then every row places its hits
-// at row_ptr[i] + (rank of dst among the row's hits): no sort, the COO comes out (src,dst)-sorted.
-// Rows whose hits did not fit the slot buffer, or with more than k_max hits, are recomputed by the
-// whole warp: exact K-smallest by (d2, j) through bisection on the bit pattern of d2 and then on j
-// among ties (storage-free), hits written unsorted and ordered by a bitonic network in place.
+// S8-S10: emit.  Thread per row in ORIGINAL order.  The search pass left sum(min(|S_i|, k_max)) per
+// 512-row tile in tile_deg, so a block gets its global edge offset by summing the totals of the
+// tiles before it (no inter-block wait), scans its own capped degrees -> CSR row_ptr, and every row
+// places its hits at row_ptr[i] + (rank of dst among the row's hits): no sort, the COO comes out
+// (src,dst)-sorted.  Rows whose hits did not fit the slot buffer, or with more than k_max hits, are
+// recomputed by the whole warp: exact K-smallest by (d2, j) through bisection on the bit pattern of
+// d2 and then on j among ties (storage-free), hits written unsorted, ordered by a bitonic network.
 // ------------------------------------------------------------------------------------------------
-constexpr int kEmitThreads = 512;
-constexpr uint64_t kFlagA = 1ull << 62, kFlagP = 2ull << 62, kValMask = (1ull << 62) - 1;
-
-__device__ __forceinline__ uint64_t ld_relaxed_u64(const uint64_t* p) {
-    uint64_t v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_relaxed_u64(uint64_t* p, uint64_t v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
 __device__ __forceinline__ void cmp_swap(int32_t* dst, float* d2, int64_t lo, int64_t hi) {
     const int32_t x = dst[lo], y = dst[hi];
     if (x > y) {
@@ -455,11 +471,10 @@ struct EmitArgs {
     const uint32_t* cell_start;
     const uint32_t* cnt;
     const int2* hits;
+    const unsigned long long* tile_deg;
     const int64_t* ev_off;        // device event offsets (n_events + 1) or NULL for one event
     int n_events;
     int64_t n_total;
-    uint64_t* tile_state;
-    uint32_t* ticket;
     int64_t* row_ptr;             // optional [n_total + 1]
     int32_t* out_src;
     int32_t* out_dst;
@@ -473,63 +488,113 @@ struct EmitArgs {
     uint32_t k_max;
 };
 
+template <int G, bool INTERIOR>
+__device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int64_t row_rp, int64_t row_ev, uint32_t row_cnt,
+                                             uint32_t cell, const float4& qa, const float4& qb, int* s_delta, int lane,
+                                             int lane_delta, uint32_t lt_mask) {
+    const float inf = __int_as_float(0x7f800000);
+    // visit(g): g(in_radius, j, d2) once per chunk, one candidate per lane
+    auto visit = [&](auto&& g) {
+        for_each_candidate_chunk<G, INTERIOR>(cell, a.bits, lane_delta, a.cell_start, s_delta, lane, [&](int cslot) {
+            float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
+            int32_t cj = -1;
+            if (cslot >= 0) {
+                ca = a.spts[2 * static_cast<int64_t>(cslot)];
+                cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
+                cj = a.sidx[cslot];
+            }
+            const float d2 = d2_pinned(qa, qb, ca, cb);
+            g(d2 <= a.r2 && cj != static_cast<int32_t>(row), cj, d2);
+        });
+    };
+    // threshold key (dthr, jthr): keep hits with (d2 bits, j) <= it.  d2 >= +0 always (the chain
+    // starts at +0 and adds squares), so bit patterns order like values.
+    uint32_t dthr = __float_as_uint(a.r2);
+    int32_t jthr = 0x7fffffff;
+    if (row_cnt > a.k_max) {
+        auto count_le = [&](uint32_t dkey, int32_t jkey) -> uint32_t {
+            uint32_t n = 0;
+            visit([&](bool in, int32_t cj, float d2) {
+                const uint32_t db = __float_as_uint(d2);
+                n += __popc(__ballot_sync(kFull, in && (db < dkey || (db == dkey && cj <= jkey))));
+            });
+            return n;
+        };
+        uint32_t dlo = 0, dhi = dthr;
+        while (dlo < dhi) {
+            const uint32_t mid = dlo + ((dhi - dlo) >> 1);
+            if (count_le(mid, 0x7fffffff) >= a.k_max) dhi = mid; else dlo = mid + 1;
+        }
+        int32_t jlo = 0, jhi = 0x7fffffff;
+        while (jlo < jhi) {
+            const int32_t mid = jlo + ((jhi - jlo) >> 1);
+            if (count_le(dlo, mid) >= a.k_max) jhi = mid; else jlo = mid + 1;
+        }
+        dthr = dlo;
+        jthr = jlo;
+    }
+    const int32_t src = static_cast<int32_t>(row - row_ev);
+    uint32_t off = 0;
+    visit([&](bool in, int32_t cj, float d2) {
+        const uint32_t db = __float_as_uint(d2);
+        const bool keep = in && (db < dthr || (db == dthr && cj <= jthr));
+        const uint32_t m = __ballot_sync(kFull, keep);
+        if (keep) {
+            const int64_t pos = row_rp + off + __popc(m & lt_mask);
+            if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = cj - static_cast<int32_t>(row_ev); a.out_d2[pos] = d2; }
+        }
+        off += __popc(m);
+    });
+    __syncwarp();
+    const int64_t kept = row_cnt < a.k_max ? row_cnt : a.k_max;
+    if (row_rp + kept <= a.capacity)                       // rows cut by the capacity stay unsorted
+        warp_sort_rows(a.out_dst + row_rp, a.out_d2 + row_rp, kept, lane);
+    __syncwarp();
+}
+
 template <int G>
-__global__ void __launch_bounds__(kEmitThreads) emit_kernel(EmitArgs a) {
-    __shared__ uint64_t s_warp[kEmitThreads / 32];
-    __shared__ uint64_t s_prefix;
-    __shared__ uint32_t s_tile;
+__global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
+    __shared__ unsigned long long s_warp[kEmitThreads / 32];
+    __shared__ unsigned long long s_prefix;
     __shared__ int s_delta[kEmitThreads / 32][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
-    if (threadIdx.x == 0) s_tile = atomicAdd(a.ticket, 1u);
-    __syncthreads();
-    const uint32_t tile = s_tile;
+    const uint32_t tile = blockIdx.x;
     const int64_t i = static_cast<int64_t>(tile) * kEmitThreads + threadIdx.x;
     const bool has = i < a.n_total;
     const uint32_t c = has ? a.cnt[i] : 0u;
     const uint32_t deg = c < a.k_max ? c : a.k_max;
+    // first hits of the row: issued early so the loads overlap the offset computation
+    const int2* h = a.hits + i * kSlot;
+    int4 h01 = make_int4(0, 0, 0, 0), h23 = h01;
+    if (c > 0) h01 = *reinterpret_cast<const int4*>(h);
+    if (c > 2) h23 = *reinterpret_cast<const int4*>(h + 2);
+    // ---- global offset of the tile = sum of the totals of the tiles before it
+    unsigned long long before = 0;
+    for (uint32_t t = threadIdx.x; t < tile; t += kEmitThreads) before += a.tile_deg[t];
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) before += __shfl_xor_sync(kFull, before, o);
     // ---- block scan of deg
-    uint64_t incl = deg;
+    uint32_t incl = deg;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const uint64_t t = __shfl_up_sync(kFull, incl, o);
+        const uint32_t t = __shfl_up_sync(kFull, incl, o);
         if (lane >= o) incl += t;
     }
-    if (lane == 31) s_warp[warp] = incl;
+    if (lane == 0) s_warp[warp] = before;
     __syncthreads();
-    uint64_t wexcl = 0, btotal = 0;
-#pragma unroll
-    for (int w = 0; w < kEmitThreads / 32; ++w) {
-        const uint64_t t = s_warp[w];
-        if (w < warp) wexcl += t;
-        btotal += t;
-    }
-    // ---- decoupled look-back for the tile's global offset
     if (warp == 0) {
-        uint64_t excl = 0;
-        if (lane == 0) st_relaxed_u64(&a.tile_state[tile], (tile == 0 ? kFlagP : kFlagA) | btotal);
-        if (tile > 0) {
-            int look = static_cast<int>(tile) - 1;
-            while (true) {
-                const int t = look - lane;
-                uint64_t st = kFlagP;                                  // virtual tile -1: prefix 0
-                if (t >= 0) {
-                    do { st = ld_relaxed_u64(&a.tile_state[t]); } while ((st >> 62) == 0);
-                }
-                const uint32_t pmask = __ballot_sync(kFull, (st >> 62) == 2);
-                const int first_p = pmask ? (__ffs(pmask) - 1) : 31;
-                uint64_t val = (lane <= first_p) ? (st & kValMask) : 0ull;
+        unsigned long long b = lane < kEmitThreads / 32 ? s_warp[lane] : 0ull;
 #pragma unroll
-                for (int o = 16; o >= 1; o >>= 1) val += __shfl_xor_sync(kFull, val, o);
-                excl += val;
-                if (pmask) break;
-                look -= 32;
-            }
-            if (lane == 0) st_relaxed_u64(&a.tile_state[tile], kFlagP | (excl + btotal));
-        }
-        if (lane == 0) s_prefix = excl;
+        for (int o = 8; o >= 1; o >>= 1) b += __shfl_xor_sync(kFull, b, o);
+        if (lane == 0) s_prefix = b;
     }
     __syncthreads();
+    if (lane == 31) s_warp[warp] = incl;                   // warp totals of deg (fits: <= 32 * k_max... use 64-bit)
+    __syncthreads();
+    unsigned long long wexcl = 0;
+#pragma unroll
+    for (int w = 0; w < kEmitThreads / 32; ++w) wexcl += (w < warp) ? s_warp[w] : 0ull;
     const int64_t rp = static_cast<int64_t>(s_prefix + wexcl + (incl - deg));      // row_ptr[i]
     // ---- CSR offsets, count, status, per-event edge offsets
     int64_t ev_base = 0;
@@ -553,24 +618,31 @@ __global__ void __launch_bounds__(kEmitThreads) emit_kernel(EmitArgs a) {
     // ---- rows that fit their slot buffer: rank by dst, place directly
     const bool big = has && (c > kSlot || c > a.k_max);
     if (has && !big && c > 0) {
-        const int2* h = a.hits + i * kSlot;
         const int32_t src = static_cast<int32_t>(i - ev_base);
-        for (uint32_t m = 0; m < c; ++m) {
-            const int2 mine = h[m];
-            uint32_t rank = 0;
-            for (uint32_t u = 0; u < c; ++u) rank += h[u].x < mine.x;
+        const int32_t eb = static_cast<int32_t>(ev_base);
+        auto put = [&](uint32_t rank, int32_t j, int32_t d2bits) {
             const int64_t pos = rp + rank;
-            if (pos < a.capacity) {
-                a.out_src[pos] = src;
-                a.out_dst[pos] = mine.x - static_cast<int32_t>(ev_base);
-                a.out_d2[pos] = __int_as_float(mine.y);
+            if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = j - eb; a.out_d2[pos] = __int_as_float(d2bits); }
+        };
+        if (c <= 4) {                                      // the common case: everything is already in registers
+            const int32_t j0 = h01.x, j1 = c > 1 ? h01.z : 0x7fffffff, j2 = c > 2 ? h23.x : 0x7fffffff, j3 = c > 3 ? h23.z : 0x7fffffff;
+            put((j1 < j0) + (j2 < j0) + (j3 < j0), j0, h01.y);
+            if (c > 1) put((j0 < j1) + (j2 < j1) + (j3 < j1), j1, h01.w);
+            if (c > 2) put((j0 < j2) + (j1 < j2) + (j3 < j2), j2, h23.y);
+            if (c > 3) put((j0 < j3) + (j1 < j3) + (j2 < j3), j3, h23.w);
+        } else {
+            for (uint32_t m = 0; m < c; ++m) {
+                const int2 mine = h[m];
+                uint32_t rank = 0;
+                for (uint32_t u = 0; u < c; ++u) rank += h[u].x < mine.x;
+                put(rank, mine.x, mine.y);
             }
         }
     }
     // ---- big rows: recompute with the whole warp
     uint32_t bigs = __ballot_sync(kFull, big);
     if (bigs == 0) return;
-    const int lane_delta = lane_row_delta<G>(lane, a.bits);
+    int lane_delta = lane_row_delta<G>(lane, a.bits);
     const uint32_t mask = (1u << a.bits) - 1u;
     for (; bigs; bigs &= bigs - 1) {
         const int bl = __ffs(bigs) - 1;
@@ -588,64 +660,8 @@ __global__ void __launch_bounds__(kEmitThreads) emit_kernel(EmitArgs a) {
             const uint32_t cd = (cell >> (d * a.bits)) & mask;
             interior = interior && cd != 0u && cd != mask;
         }
-        const float inf = __int_as_float(0x7f800000);
-        // visit(g): g(hit_candidate_lane, j, d2) once per chunk with the in-radius test applied
-        auto visit = [&](auto&& g) {
-            for_each_candidate_chunk<G>(cell, interior, a.bits, lane_delta, a.cell_start, s_delta[warp], lane, [&](int cslot) {
-                float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
-                int32_t cj = -1;
-                if (cslot >= 0) {
-                    ca = a.spts[2 * static_cast<int64_t>(cslot)];
-                    cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
-                    cj = a.sidx[cslot];
-                }
-                const float d2 = d2_pinned(qa, qb, ca, cb);
-                g(d2 <= a.r2 && cj != static_cast<int32_t>(row), cj, d2);
-            });
-        };
-        // threshold key (dthr, jthr): keep hits with (d2 bits, j) <= it.  d2 >= +0 always (the chain
-        // starts at +0 and adds squares), so bit patterns order like values.
-        uint32_t dthr = __float_as_uint(a.r2);
-        int32_t jthr = 0x7fffffff;
-        if (row_cnt > a.k_max) {
-            auto count_le = [&](uint32_t dkey, int32_t jkey) -> uint32_t {
-                uint32_t n = 0;
-                visit([&](bool in, int32_t cj, float d2) {
-                    const uint32_t db = __float_as_uint(d2);
-                    n += __popc(__ballot_sync(kFull, in && (db < dkey || (db == dkey && cj <= jkey))));
-                });
-                return n;
-            };
-            uint32_t dlo = 0, dhi = dthr;
-            while (dlo < dhi) {
-                const uint32_t mid = dlo + ((dhi - dlo) >> 1);
-                if (count_le(mid, 0x7fffffff) >= a.k_max) dhi = mid; else dlo = mid + 1;
-            }
-            int32_t jlo = 0, jhi = 0x7fffffff;
-            while (jlo < jhi) {
-                const int32_t mid = jlo + ((jhi - jlo) >> 1);
-                if (count_le(dlo, mid) >= a.k_max) jhi = mid; else jlo = mid + 1;
-            }
-            dthr = dlo;
-            jthr = jlo;
-        }
-        const int32_t src = static_cast<int32_t>(row - row_ev);
-        uint32_t off = 0;
-        visit([&](bool in, int32_t cj, float d2) {
-            const uint32_t db = __float_as_uint(d2);
-            const bool keep = in && (db < dthr || (db == dthr && cj <= jthr));
-            const uint32_t m = __ballot_sync(kFull, keep);
-            if (keep) {
-                const int64_t pos = row_rp + off + __popc(m & lt_mask);
-                if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = cj - static_cast<int32_t>(row_ev); a.out_d2[pos] = d2; }
-            }
-            off += __popc(m);
-        });
-        __syncwarp();
-        const int64_t kept = row_cnt < a.k_max ? row_cnt : a.k_max;
-        if (row_rp + kept <= a.capacity)                       // rows cut by the capacity stay unsorted
-            warp_sort_rows(a.out_dst + row_rp, a.out_d2 + row_rp, kept, lane);
-        __syncwarp();
+        if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
+        else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
     }
 }
 
