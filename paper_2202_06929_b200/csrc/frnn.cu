@@ -59,7 +59,7 @@ struct Layout {
     int rows_per_block;
     int64_t scan_blocks;
     size_t off_cells, off_tiles, off_counters, zero_bytes;
-    size_t off_pcell, off_prank, off_spts, off_sidx, off_cnt, off_evoff, off_segs, off_hits;
+    size_t off_pcell, off_prank, off_spts, off_sidx, off_scell, off_skey, off_cnt, off_evoff, off_hits;
     size_t total;
 };
 
@@ -75,48 +75,21 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     L.emit_tiles = (n_total + kEmitThreads - 1) / kEmitThreads;
     size_t o = 0;
     L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_entries + 8) * 4);
-    L.off_tiles = o;    o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8);
-    L.off_counters = o; o = align_up(o + 64);          // [0..7] cursor (u64), [8..11] emit ticket
-    L.zero_bytes = o;
+    L.off_tiles = o;    o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8 * kDegSlices);
+    L.off_counters = o; o = align_up(o + 64);          // [0..3] cursor of the cell scan (u32)
     const size_t n = static_cast<size_t>(n_total > 0 ? n_total : 1);
-    const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
+    L.off_cnt = o;      o = align_up(o + n * 4);       // zeroed: the search pass counts with atomics
+    L.zero_bytes = o;
     L.off_pcell = o;  o = align_up(o + n * 4);
     L.off_prank = o;  o = align_up(o + n * 4);
     L.off_spts = o;   o = align_up(o + n * 32);
     L.off_sidx = o;   o = align_up(o + n * 4);
-    L.off_cnt = o;    o = align_up(o + n * 4);
+    L.off_scell = o;  o = align_up(o + n * 4);
+    L.off_skey = o;   o = align_up(o + n * 4);
     L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
-    L.off_segs = o;   o = align_up(o + static_cast<size_t>(max_segs > 0 ? max_segs : 1) * sizeof(Segment));
     L.off_hits = o;   o = align_up(o + n * kSlot * sizeof(int2));
     L.total = o;
     return L;
-}
-
-int g_num_sms = 0;
-int num_sms() {
-    if (!g_num_sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-    }
-    return g_num_sms;
-}
-
-template <int G>
-cudaError_t launch_search(const SearchArgs& a, int64_t max_segs, cudaStream_t st) {
-    static int blocks_per_sm = 0;
-    if (!blocks_per_sm) {
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, search_kernel<G>, kSearchWarps * 32, 0) != cudaSuccess ||
-            blocks_per_sm < 1)
-            blocks_per_sm = 1;
-    }
-    int64_t blocks = (max_segs + kSearchWarps - 1) / kSearchWarps;
-    const int64_t resident = static_cast<int64_t>(num_sms()) * blocks_per_sm;
-    if (blocks > resident) blocks = resident;
-    if (blocks < 1) blocks = 1;
-    search_kernel<G><<<static_cast<unsigned>(blocks), kSearchWarps * 32, 0, st>>>(a);
-    ++t_launches;
-    return cudaGetLastError();
 }
 
 #define FRNN_DISPATCH_G(G_, EXPR)          \
@@ -172,14 +145,15 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     char* ws = static_cast<char*>(c.workspace);
     uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
     unsigned long long* tile_deg = reinterpret_cast<unsigned long long*>(ws + L.off_tiles);
-    unsigned long long* cursor = reinterpret_cast<unsigned long long*>(ws + L.off_counters);
+    unsigned int* cursor = reinterpret_cast<unsigned int*>(ws + L.off_counters);
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
     int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
+    uint32_t* scell = reinterpret_cast<uint32_t*>(ws + L.off_scell);
+    uint32_t* skey = reinterpret_cast<uint32_t*>(ws + L.off_skey);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
     int64_t* ev_off = reinterpret_cast<int64_t*>(ws + L.off_evoff);
-    Segment* segs = reinterpret_cast<Segment*>(ws + L.off_segs);
     int2* hits = reinterpret_cast<int2*>(ws + L.off_hits);
     const float4* pts = reinterpret_cast<const float4*>(c.points);
     const int G = c.grid_dims, bits = c.grid_bits;
@@ -209,19 +183,19 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank)));
     ++t_launches; CK(cudaGetLastError());
     mark(1, st);
-    FRNN_DISPATCH_G(G, (cell_scan_kernel<GG><<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries,
-                                                                                                           L.rows_per_block, bits, segs, cursor)));
+    cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor);
     ++t_launches; CK(cudaGetLastError());
     mark(2, st);
-    scatter_kernel<<<row_blocks, 256, 0, st>>>(pts, n_total, cells, pcell, prank, spts, sidx);
+    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, scell, skey)));
     ++t_launches; CK(cudaGetLastError());
     mark(3, st);
 
     SearchArgs sa;
-    sa.spts = spts; sa.sidx = sidx; sa.cell_start = cells; sa.segs = segs; sa.cursor = cursor; sa.cnt = cnt; sa.hits = hits;
-    sa.tile_deg = tile_deg; sa.r2 = r2; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
-    const int64_t max_segs = n_total < L.n_cells ? n_total : L.n_cells;
-    FRNN_DISPATCH_G(G, CK((launch_search<GG>(sa, max_segs, st))));
+    sa.spts = spts; sa.sidx = sidx; sa.scell = scell; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
+    sa.tile_deg = tile_deg; sa.n_total = n_total; sa.r2 = r2; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
+    const unsigned search_blocks = static_cast<unsigned>((n_total + kSearchThreads - 1) / kSearchThreads);
+    FRNN_DISPATCH_G(G, (search_kernel<GG><<<search_blocks, kSearchThreads, 0, st>>>(sa)));
+    ++t_launches; CK(cudaGetLastError());
     mark(4, st);
 
     EmitArgs ea;

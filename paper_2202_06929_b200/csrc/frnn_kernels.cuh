@@ -37,7 +37,9 @@ constexpr float kCoordClamp = 32768.0f;
 __device__ __forceinline__ uint32_t cell_coord(float x, float inv_cell, uint32_t mask) {
     float a = __fmul_rn(x, inv_cell);
     a = fminf(fmaxf(a, -kCoordClamp), kCoordClamp);   // NaN -> -clamp: never out of bounds
-    return static_cast<uint32_t>(__float2int_rd(a)) & mask;
+    // + half the extent: data centred on the origin sits in the middle of [0, 2^bits), so the seam of
+    // the torus (cells 0 and 2^bits-1 are neighbours) is met only by points beyond +-2^(bits-1) cells
+    return static_cast<uint32_t>(__float2int_rd(a) + static_cast<int>((mask + 1u) >> 1)) & mask;
 }
 
 template <int G>
@@ -51,6 +53,26 @@ __device__ __forceinline__ uint32_t cell_of_point(const float4& a, const float4&
 }
 
 __device__ __forceinline__ uint32_t padded(uint32_t lin, int bits) { return lin + (lin >> bits); }
+
+// Filter key of a point: the cell coordinate (same side, modulo 64) of up to four coordinates that
+// are NOT binned (dims G..G+3), one per byte.  Two points within r of each other differ by at most
+// one cell in every coordinate (same argument as for the grid), so  |q_a - q_c| mod 64 in {0, 1, 63}
+// per field is a NECESSARY condition for an edge: candidates failing it are dropped without touching
+// their coordinates.  With A = key(query) + 0x81818181 the bytewise difference A - key(candidate)
+// never borrows across bytes (129 + q_a - q_c is in [66, 192]) and its low six bits per byte are
+// (q_a - q_c + 1) mod 64: the pair passes iff these are all <= 3 (3 is a harmless false positive).
+constexpr uint32_t kKeyBias = 0x81818181u;
+constexpr uint32_t kKeyReject = 0x3c3c3c3cu;
+
+template <int G>
+__device__ __forceinline__ uint32_t key_of_point(const float4& a, const float4& b, float inv_cell) {
+    const float x[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+    uint32_t key = 0;
+#pragma unroll
+    for (int f = 0; f < 4; ++f)
+        if (G + f < kDim) key |= cell_coord(x[G + f], inv_cell, 63u) << (8 * f);
+    return key;
+}
 
 // DESIGN.md R3: the pinned fp32 order.  Explicit rounding intrinsics: nvcc may not contract,
 // reassociate or reorder them.  Each lane runs the whole chain for one (query, candidate) pair.
@@ -102,55 +124,50 @@ __global__ void __launch_bounds__(256) bin_kernel(const float4* __restrict__ pts
     float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
     if (G > 4) b = pts[2 * i + 1];
     const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
-    const uint32_t pid = padded(cell_of_point<G>(a, b, ev, inv_cell, bits), bits);
-    pcell[i] = pid;
-    prank[i] = atomicAdd(&cell_count[pid], 1u);
+    const uint32_t lin = cell_of_point<G>(a, b, ev, inv_cell, bits);
+    pcell[i] = lin;
+    prank[i] = atomicAdd(&cell_count[padded(lin, bits)], 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
 // S4: counting-sort scatter.  Order inside a cell is the (arbitrary) atomic order; the final
 // result does not depend on it because every row is ordered by dst at the end.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) scatter_kernel(const float4* __restrict__ pts, int64_t n_total,
+template <int G>
+__global__ void __launch_bounds__(256) scatter_kernel(const float4* __restrict__ pts, int64_t n_total, int bits, float inv_cell,
                                                       const uint32_t* __restrict__ cell_start,
                                                       const uint32_t* __restrict__ pcell,
                                                       const uint32_t* __restrict__ prank,
-                                                      float4* __restrict__ spts, int32_t* __restrict__ sidx) {
+                                                      float4* __restrict__ spts, int32_t* __restrict__ sidx,
+                                                      uint32_t* __restrict__ scell, uint32_t* __restrict__ skey) {
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i >= n_total) return;
-    const uint32_t s = cell_start[pcell[i]] + prank[i];
+    const uint32_t lin = pcell[i];
+    const uint32_t s = cell_start[padded(lin, bits)] + prank[i];
     const float4 a = pts[2 * i], b = pts[2 * i + 1];
     spts[2 * static_cast<int64_t>(s)] = a;
     spts[2 * static_cast<int64_t>(s) + 1] = b;
     sidx[s] = static_cast<int32_t>(i);
+    scell[s] = lin;
+    skey[s] = key_of_point<G>(a, b, inv_cell);
 }
 
 // ------------------------------------------------------------------------------------------------
 // S3: cell starts.  Each block owns a few WHOLE padded rows of the table (about 4096 entries),
-// computes its total, reserves its range of the cell-ordered copy with ONE 64-bit atomicAdd that
-// packs (occupied cells << 32 | points), then scans its rows in strips of 1024.  Blocks land in
-// arrival order: no inter-block wait, and since a run only ever reads start[lo] and start[hi+1] of
-// one row (the padding entry holds the row's end) nothing depends on the order of the blocks.
-// The block also appends its occupied cells to the segment list (same atomic).
+// computes its total, reserves its range of the cell-ordered copy with ONE atomicAdd, then writes the
+// exclusive scan of its entries.  Blocks land in arrival order: no inter-block wait, and since a run
+// only ever reads start[lo] and start[hi+1] of one row (the padding entry holds the row's end)
+// nothing depends on the order of the blocks.
 // ------------------------------------------------------------------------------------------------
-struct Segment {          // one occupied cell: the unit of work of the search kernel
-    uint32_t cell;        // linear cell id (event index in the high bits)
-    uint32_t start;       // first slot in the cell-ordered copy
-    uint32_t len;         // points in the cell
-    uint32_t interior;    // 1 if no coordinate of the cell is 0 or 2^bits-1 (no wrap among its neighbours)
-};
-
 constexpr int kCellThreads = 1024;
 constexpr int kCellTile = 4 * kCellThreads;      // table entries per block (upper bound)
 
 // A block owns `rows_per_block` whole padded rows = rows_per_block * (2^bits + 1) <= kCellTile
 // entries (a multiple of 4, so every thread moves one aligned uint4).
-template <int G>
 __global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __restrict__ cells, int64_t n_entries, int rows_per_block,
-                                                                 int bits, Segment* __restrict__ segs,
-                                                                 unsigned long long* __restrict__ cursor) {
-    __shared__ uint32_t s_pts[32], s_occ[32];
-    __shared__ unsigned long long s_base;
+                                                                 int bits, unsigned int* __restrict__ cursor) {
+    __shared__ uint32_t s_pts[32];
+    __shared__ uint32_t s_base;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t row_len = (1u << bits) + 1u;
     const uint32_t blk_entries = static_cast<uint32_t>(rows_per_block) * row_len;
@@ -160,61 +177,31 @@ __global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __res
     uint4 v = make_uint4(0u, 0u, 0u, 0u);
     if (act) v = *reinterpret_cast<const uint4*>(cells + blk_base + local);
     const uint32_t tp = v.x + v.y + v.z + v.w;
-    const uint32_t to = (v.x != 0u) + (v.y != 0u) + (v.z != 0u) + (v.w != 0u);
-    uint32_t ip = tp, io = to;                                                 // inclusive warp scans
+    uint32_t ip = tp;                                                          // inclusive warp scan
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t a = __shfl_up_sync(kFull, ip, o), b = __shfl_up_sync(kFull, io, o);
-        if (lane >= o) { ip += a; io += b; }
+        const uint32_t t = __shfl_up_sync(kFull, ip, o);
+        if (lane >= o) ip += t;
     }
-    if (lane == 31) { s_pts[warp] = ip; s_occ[warp] = io; }
+    if (lane == 31) s_pts[warp] = ip;
     __syncthreads();
     if (warp == 0) {
-        const uint32_t wp = s_pts[lane], wo = s_occ[lane];
-        uint32_t sp = wp, so = wo;
+        const uint32_t wp = s_pts[lane];
+        uint32_t sp = wp;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t a = __shfl_up_sync(kFull, sp, o), b = __shfl_up_sync(kFull, so, o);
-            if (lane >= o) { sp += a; so += b; }
+            const uint32_t t = __shfl_up_sync(kFull, sp, o);
+            if (lane >= o) sp += t;
         }
         s_pts[lane] = sp - wp;                                                 // exclusive warp offsets
-        s_occ[lane] = so - wo;
-        if (lane == 31) {
-            const unsigned long long total = (static_cast<unsigned long long>(so) << 32) | sp;
-            s_base = total ? atomicAdd(cursor, total) : 0ull;
-        }
+        if (lane == 31) s_base = sp ? atomicAdd(cursor, sp) : 0u;
     }
     __syncthreads();
     if (!act) return;
-    const unsigned long long base = s_base;
-    uint32_t p = static_cast<uint32_t>(base) + s_pts[warp] + (ip - tp);
-    uint32_t oc = static_cast<uint32_t>(base >> 32) + s_occ[warp] + (io - to);
-    const uint32_t cnt[4] = {v.x, v.y, v.z, v.w};
+    const uint32_t p = s_base + s_pts[warp] + (ip - tp);
     uint4 out;
     out.x = p; out.y = p + v.x; out.z = out.y + v.y; out.w = out.z + v.z;
     *reinterpret_cast<uint4*>(cells + blk_base + local) = out;
-    if (to) {
-        const uint32_t mask = (1u << bits) - 1u;
-        const float inv_row = 1.0f / static_cast<float>(row_len);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (cnt[k]) {
-                // table index -> linear id: drop the padding entries of the rows before this one
-                const uint32_t e = local + k;
-                const uint32_t row_local = __float2uint_rz((static_cast<float>(e) + 0.5f) * inv_row);     // e / row_len, e < 4096
-                const uint32_t lin = static_cast<uint32_t>(blk_base + e) - (blockIdx.x * static_cast<uint32_t>(rows_per_block) + row_local);
-                bool interior = true;
-#pragma unroll
-                for (int d = 0; d < G; ++d) {
-                    const uint32_t c = (lin >> (d * bits)) & mask;
-                    interior = interior && c != 0u && c != mask;
-                }
-                segs[oc] = Segment{lin, p, cnt[k], interior ? 1u : 0u};
-                ++oc;
-            }
-            p += cnt[k];
-        }
-    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -319,108 +306,200 @@ __device__ __forceinline__ void for_each_candidate_chunk(uint32_t cell, int bits
 }
 
 // ------------------------------------------------------------------------------------------------
-// S6/S7: the single search pass.  One warp per segment (occupied cell), persistent grid-stride
-// over the segment list.  Queries = the cell's points (<= 32 per pass) staged in shared memory and
-// read back as broadcasts; candidates = one per lane per chunk (2 x 128-bit loads of the 32-byte
-// row).  Lane q keeps the running hit count of query q.  Every hit (j, d2) is appended to the
-// query's slot buffer hits[row * kSlot + pos] (pos < kSlot); the count keeps running beyond kSlot,
-// which tells emit_kernel to resolve that row by recomputation.
+// S5-S7: the single search pass, ONE THREAD PER QUERY in cell order (thread = slot of the
+// cell-ordered copy), so the lanes of a warp sit in the same or adjacent cells and their loads of
+// the table, the keys and the candidate rows fall into the same few cache lines.
+//
+// Every unordered pair is evaluated ONCE.  d2 is bitwise symmetric (x - y = -(y - x) exactly, the
+// squares and the FMA chain are identical), so a query only visits the "forward" half of its
+// neighbourhood: cell offsets (o_0 .. o_{G-1}) that are lexicographically positive, plus the slots
+// after its own in its own cell -- 13.5 of the 27 runs at G = 4 -- and a hit is appended to BOTH
+// rows' slot buffers (position from an atomic counter per row).
+//
+// Phase 1 (filter).  Neighbour rows are visited in sub-batches of 3 rows (the offsets of coordinate
+// G-2, unrolled).  A run is [start[row+lo], start[row+hi+1]); its first kBatch candidates are tested
+// straight-line -- 3 x kBatch independent 4-byte key loads in flight per thread -- and longer runs
+// finish in batches of kBatch.  Only the filter key of a candidate is read here (see key_of_point):
+// ~85 % of the candidates of a tracking event are rejected with 3 integer instructions and 4 bytes
+// of traffic.  Survivors go on the thread's queue (its own column of a shared-memory array; the
+// store is unconditional, the queue pointer advances only for survivors: no branch).
+// Phase 2 (evaluate) drains the queue: 32-byte row + index loads (next row in flight while the
+// current one is evaluated), the whole R3 chain per lane.  Hit (i, j, d2): pos = cnt[i]++ and
+// hits[i * kSlot + pos] = (j, d2) if pos < kSlot, the same for j; the counts keep running beyond
+// kSlot, which tells emit_kernel to resolve that row by recomputation.  min(cnt, k_max) is the
+// number of increments that found a value < k_max, so the per-tile capped degree totals emit_kernel
+// needs are accumulated exactly by the same increments.
+// Lanes whose cell touches the seam of the torus in the last coordinate (only points beyond
+// +-2^(bits-1) cells from the origin) also filter the wrapped cell.
 // ------------------------------------------------------------------------------------------------
-constexpr int kSearchWarps = 8;
-// ptxas caps registers from the launch bounds: 5 resident blocks of 256 threads = 48 registers.
+constexpr int kSearchThreads = 128;
 #ifndef FRNN_SEARCH_MIN_BLOCKS
-#define FRNN_SEARCH_MIN_BLOCKS 5
+#define FRNN_SEARCH_MIN_BLOCKS 7       // 7 x 128 threads: 72 registers per thread; 7 x 148 blocks >= one 120k-point event
 #endif
+constexpr int kBatch = 4;              // candidates of a run tested per batch
+constexpr int kQueue = 32;             // survivor queue entries per thread (>= 2 * 3 * kBatch)
 constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
 constexpr int kEmitThreads = 512;      // rows per emit tile
+constexpr int kDegSlices = 32;         // copies of every per-tile degree counter (spreads same-address atomics)
 
 struct SearchArgs {
     const float4* spts;
     const int32_t* sidx;          // slot -> global row index
+    const uint32_t* scell;        // slot -> linear cell id
+    const uint32_t* skey;         // slot -> filter key
     const uint32_t* cell_start;
-    const Segment* segs;
-    const unsigned long long* cursor;   // high 32 bits = number of segments
-    uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index
+    uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index (zeroed)
     int2* hits;                   // [n_total * kSlot] (j global, d2 bits)
-    unsigned long long* tile_deg; // [ceil(n_total / kEmitThreads)] sum of min(|S_i|, k_max) per emit tile (zeroed)
+    unsigned long long* tile_deg; // [ceil(n_total / kEmitThreads) * kDegSlices] partial sums of min(|S_i|, k_max) per emit tile (zeroed)
+    int64_t n_total;
     float r2;
     int bits;
     uint32_t k_max;
 };
 
-template <int G, bool INTERIOR>
-__device__ __forceinline__ void search_segment(const SearchArgs& a, const Segment& seg, float4* q, int* s_delta, int lane,
-                                               int lane_delta, uint32_t lt_mask) {
-    const float inf = __int_as_float(0x7f800000);
-    for (uint32_t q0 = 0; q0 < seg.len; q0 += 32) {
-        const int nq = min(32u, seg.len - q0);
-        const uint32_t first_slot = seg.start + q0;
-        const bool has = lane < nq;
-        int32_t my_row = 0;
-        uint32_t my_cnt = 0;
-        __syncwarp();
-        if (has) {
-            q[2 * lane] = a.spts[2 * static_cast<int64_t>(first_slot + lane)];
-            q[2 * lane + 1] = a.spts[2 * static_cast<int64_t>(first_slot + lane) + 1];
-            my_row = a.sidx[first_slot + lane];
-        }
-        __syncwarp();
-        for_each_candidate_chunk<G, INTERIOR>(seg.cell, a.bits, lane_delta, a.cell_start, s_delta, lane, [&](int cslot) {
-            float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);   // no candidate: d2 = inf
-            int32_t cj = 0;
-            if (cslot >= 0) {
-                ca = a.spts[2 * static_cast<int64_t>(cslot)];
-                cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
-                cj = a.sidx[cslot];
-            }
-            const int self_q = cslot - static_cast<int>(first_slot);   // the query this candidate IS (if in [0, nq))
-            for (int qi = 0; qi < nq; ++qi) {
-                const float d2 = d2_pinned(q[2 * qi], q[2 * qi + 1], ca, cb);
-                const bool hit = d2 <= a.r2 && self_q != qi;
-                const uint32_t m = __ballot_sync(kFull, hit);
-                if (m) {
-                    const uint32_t base = __shfl_sync(kFull, my_cnt, qi);
-                    const int32_t row = __shfl_sync(kFull, my_row, qi);
-                    if (hit) {
-                        const uint32_t pos = base + __popc(m & lt_mask);
-                        if (pos < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + pos] = make_int2(cj, __float_as_int(d2));
-                    }
-                    if (lane == qi) my_cnt += __popc(m);
-                }
-            }
-        });
-        if (has) {
-            a.cnt[my_row] = my_cnt;
-            // per-tile degree totals: emit_kernel turns them into its global offsets without any
-            // inter-block wait
-            if (my_cnt) atomicAdd(&a.tile_deg[my_row / kEmitThreads], static_cast<unsigned long long>(my_cnt < a.k_max ? my_cnt : a.k_max));
-        }
-    }
-}
-
 template <int G>
-__global__ void __launch_bounds__(kSearchWarps * 32, FRNN_SEARCH_MIN_BLOCKS) search_kernel(SearchArgs a) {
-    __shared__ float4 s_q[kSearchWarps][64];
-    __shared__ int s_delta[kSearchWarps][32];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-    const uint32_t n_segs = static_cast<uint32_t>(*a.cursor >> 32);
-    const uint32_t stride = gridDim.x * kSearchWarps;
-    int lane_delta = lane_row_delta<G>(lane, a.bits);
-    asm volatile("" : "+r"(lane_delta));                  // keep it in a register: do not recompute per segment
-    uint32_t sg = blockIdx.x * kSearchWarps + warp;
-    if (sg >= n_segs) return;
-    Segment seg = a.segs[sg];
-    while (true) {
-        const uint32_t nxt = sg + stride;
-        Segment seg_next = seg;
-        if (nxt < n_segs) seg_next = a.segs[nxt];         // prefetch: the load overlaps this segment's work
-        if (seg.interior) search_segment<G, true>(a, seg, s_q[warp], s_delta[warp], lane, lane_delta, lt_mask);
-        else              search_segment<G, false>(a, seg, s_q[warp], s_delta[warp], lane, lane_delta, lt_mask);
-        if (nxt >= n_segs) break;
-        sg = nxt;
-        seg = seg_next;
+__global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search_kernel(SearchArgs a) {
+    constexpr int NU = G >= 2 ? 3 : 1;                    // unrolled offsets of coordinate G-2
+    constexpr int NB = pow3(G >= 2 ? G - 2 : 0);          // sub-batches: offsets of coordinates 0..G-3 (dim 0 most significant)
+    constexpr int MID = (NB - 1) / 2;                     // the sub-batch with all-zero offsets
+    __shared__ uint32_t s_queue[kQueue + 1][kSearchThreads];
+    const int tid = threadIdx.x;
+    const int64_t s64 = static_cast<int64_t>(blockIdx.x) * kSearchThreads + tid;
+    if (s64 >= a.n_total) return;                         // no block-wide barrier below
+    const uint32_t s = static_cast<uint32_t>(s64);
+    const float4 qa = a.spts[2 * s64], qb = a.spts[2 * s64 + 1];
+    const int32_t my_row = a.sidx[s];
+    const uint32_t cell = a.scell[s];
+    const uint32_t key_a = a.skey[s] + kKeyBias;
+    const int bits = a.bits;
+    const uint32_t mask = (1u << bits) - 1u;
+    const uint32_t c_last = cell & mask;
+    const uint32_t lo = c_last ? c_last - 1u : 0u, hi = c_last < mask ? c_last + 1u : mask;
+    const bool seam = c_last == 0u || c_last == mask;
+    const uint32_t wrap_cell = c_last == 0u ? mask : 0u;
+    const uint32_t deg_slice = blockIdx.x & (kDegSlices - 1);
+    uint32_t own_deg = 0;                                 // increments of cnt[my_row] made here that found a value < k_max
+    uint32_t* qp = &s_queue[0][tid];                      // next free queue entry
+    uint32_t* const q0 = qp;
+    constexpr int kQStride = kSearchThreads;              // in words
+
+    auto test = [&](const float4& ca, const float4& cb, int32_t cj) {
+        const float d2 = d2_pinned(qa, qb, ca, cb);
+        if (d2 <= a.r2) {
+            const int d2b = __float_as_int(d2);
+            const uint32_t p = atomicAdd(&a.cnt[my_row], 1u);
+            const uint32_t q = atomicAdd(&a.cnt[cj], 1u);
+            if (p < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + p] = make_int2(cj, d2b);
+            if (q < kSlot) a.hits[static_cast<int64_t>(cj) * kSlot + q] = make_int2(my_row, d2b);
+            own_deg += p < a.k_max;
+            if (q < a.k_max) atomicAdd(&a.tile_deg[(cj / kEmitThreads) * kDegSlices + deg_slice], 1ull);
+        }
+    };
+    // phase 2: evaluate the queued survivors (never the query itself)
+    auto drain = [&]() {
+        const int qn = static_cast<int>(qp - q0) / kQStride;
+        qp = q0;
+        if (qn == 0) return;
+        uint32_t j = q0[0];
+        float4 xa = a.spts[2 * static_cast<int64_t>(j)], xb = a.spts[2 * static_cast<int64_t>(j) + 1];
+        int32_t xj = a.sidx[j];
+        float4 ya, yb;
+        int32_t yj;
+        int i = 1;
+        while (true) {
+            if (i < qn) { j = q0[i * kQStride]; ya = a.spts[2 * static_cast<int64_t>(j)]; yb = a.spts[2 * static_cast<int64_t>(j) + 1]; yj = a.sidx[j]; }
+            test(xa, xb, xj);
+            if (++i > qn) break;
+            if (i < qn) { j = q0[i * kQStride]; xa = a.spts[2 * static_cast<int64_t>(j)]; xb = a.spts[2 * static_cast<int64_t>(j) + 1]; xj = a.sidx[j]; }
+            test(ya, yb, yj);
+            if (++i > qn) break;
+        }
+    };
+    // phase 1 for one candidate slot: branch-free push (the entry is only kept if the pointer advances);
+    // the caller guarantees one free entry
+    auto filter = [&](bool valid, uint32_t j, uint32_t key_c) {
+        const bool pass = valid && ((key_a - key_c) & kKeyReject) == 0u;
+        *qp = j;
+        qp += pass ? kQStride : 0;
+    };
+    // padded table index of cell 0 of the neighbour row: coordinates 0..G-3 offset by the base-3 digits
+    // of b (coordinate 0 most significant), coordinate G-2 by u - 1 (wrapped)
+    auto row_of = [&](int b, int u) -> uint32_t {
+        uint32_t base = cell >> (G * bits);               // event index
+#pragma unroll
+        for (int d = 0; d < G - 1; ++d) {
+            int o;
+            if (d < G - 2) o = (b / pow3(G - 3 - d)) % 3 - 1; else o = u - 1;
+            const uint32_t cd = (cell >> ((G - 1 - d) * bits)) & mask;
+            base = (base << bits) | ((cd + static_cast<uint32_t>(o)) & mask);
+        }
+        return (base << bits) + base;                     // padded(base << bits)
+    };
+
+    for (int b = MID; b < NB; ++b) {
+        const bool zero = b == MID;                       // row offsets 0 in coordinates 0..G-3
+        uint32_t rs[NU], re[NU];
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const int uu = G >= 2 ? u : 1;
+            const uint32_t row = row_of(b, uu);
+            rs[u] = a.cell_start[row + lo];
+            re[u] = a.cell_start[row + hi + 1u];
+            if (zero && uu == 1) rs[u] = s + 1u;          // own row: the slots after mine (my cell and the next one)
+            if (zero && uu == 0) re[u] = rs[u];           // backward row: its queries come to me
+        }
+        if (qp - q0 > (kQueue - NU * kBatch) * kQStride) drain();
+        uint32_t kc[NU][kBatch];
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const uint32_t* kp = a.skey + rs[u];          // one 64-bit base per run, immediate offsets
+            const uint32_t len = re[u] - rs[u];
+#pragma unroll
+            for (int v = 0; v < kBatch; ++v) {
+                kc[u][v] = 0u;
+                if (static_cast<uint32_t>(v) < len) kc[u][v] = kp[v];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const uint32_t len = re[u] - rs[u];
+#pragma unroll
+            for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, rs[u] + v, kc[u][v]);
+        }
+        // runs longer than kBatch, and the wrapped cell of lanes on the seam of the torus: batches of
+        // kBatch in ONE copy of the loop (the run is picked with selects so rs/re stay in registers)
+        for (int t = 0; t < (seam ? 2 * NU : NU); ++t) {
+            const int u = t < NU ? t : t - NU;
+            uint32_t j0 = rs[0] + kBatch, j1 = re[0];
+#pragma unroll
+            for (int w = 1; w < NU; ++w)
+                if (u == w) { j0 = rs[w] + kBatch; j1 = re[w]; }
+            if (t >= NU) {
+                const int uu = G >= 2 ? u : 1;
+                const uint32_t row = row_of(b, uu);
+                j0 = a.cell_start[row + wrap_cell];
+                j1 = a.cell_start[row + wrap_cell + 1u];
+                // own row: only the cell after mine is forward; backward row: nothing
+                if (zero && (uu == 0 || (uu == 1 && c_last != mask))) j1 = j0;
+            }
+            for (; j0 < j1; j0 += kBatch) {
+                if (qp - q0 > (kQueue - kBatch) * kQStride) drain();
+                const uint32_t* kp = a.skey + j0;
+                const uint32_t len = j1 - j0;
+                uint32_t kr[kBatch];
+#pragma unroll
+                for (int v = 0; v < kBatch; ++v) {
+                    kr[v] = 0u;
+                    if (static_cast<uint32_t>(v) < len) kr[v] = kp[v];
+                }
+#pragma unroll
+                for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, j0 + v, kr[v]);
+            }
+        }
     }
+    drain();
+    // per-tile degree totals: emit_kernel turns them into its global offsets without any inter-block wait
+    if (own_deg) atomicAdd(&a.tile_deg[(my_row / kEmitThreads) * kDegSlices + deg_slice], static_cast<unsigned long long>(own_deg));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -571,7 +650,7 @@ __global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
     if (c > 2) h23 = *reinterpret_cast<const int4*>(h + 2);
     // ---- global offset of the tile = sum of the totals of the tiles before it
     unsigned long long before = 0;
-    for (uint32_t t = threadIdx.x; t < tile; t += kEmitThreads) before += a.tile_deg[t];
+    for (uint32_t t = threadIdx.x; t < tile * kDegSlices; t += kEmitThreads) before += a.tile_deg[t];
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) before += __shfl_xor_sync(kFull, before, o);
     // ---- block scan of deg
