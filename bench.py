@@ -288,8 +288,11 @@ def main() -> None:
     achieved = alg_bytes / (dom_us * 1e-6) / 1e9 if dom_us and dom_us == dom_us else float("nan")
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get(dom)
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:      # ncu dram bytes per launch (see profiles/traffic.md)
+            for row in f.read().splitlines()[1:]:
+                k, v = row.split(",")[:2]
+                if k == dom:
+                    traffic = int(v)
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
