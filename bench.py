@@ -183,6 +183,7 @@ def main() -> None:
     ap.add_argument("--cpu-events", type=int, default=24, help="events the cpu_baseline leg runs the oracle on")
     ap.add_argument("--e2e-steps", type=int, default=1000)
     ap.add_argument("--profile-steps", type=int, default=200)
+    ap.add_argument("--timeline-steps", type=int, default=100)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -274,6 +275,24 @@ def main() -> None:
     F.frnn_set_profiling(False)
     phases_us = {k: 1e3 * v / max(args.profile_steps, 1) for k, v in phases.items()}
 
+    # in-graph timeline (%globaltimer stamps written by the kernels themselves; the graph replay is untouched)
+    timeline_us = None
+    if args.timeline_steps > 0:
+        F.frnn_set_profiling(2)
+        acc = {}
+        with torch.cuda.stream(stream):
+            for rep in range(args.timeline_steps):
+                for k in range(8):                      # back to back, as in the timed loop; the stamps of the last call stay
+                    step(rep * 8 + k)
+                stream.synchronize()
+                for name, (b0, e0) in F.frnn_get_timeline(shared, n, 1).items():
+                    a = acc.setdefault(name, [0.0, 0.0])
+                    a[0] += b0
+                    a[1] += e0
+        F.frnn_set_profiling(0)
+        timeline_us = {k: {"begin": v[0] / args.timeline_steps, "end": v[1] / args.timeline_steps,
+                           "dur": (v[1] - v[0]) / args.timeline_steps} for k, v in acc.items()}
+
     # roofline of the dominant kernel
     peak, peak_src = measured_peak()
     dims, bits = F.frnn_get_grid(n, 1)
@@ -346,7 +365,7 @@ def main() -> None:
                        "l2": f"inputs and outputs rotate over {len(seeds)} events ({len(seeds) * n * 32 / 1e6:.0f} MB in + "
                              f"{len(seeds) * cap * 12 / 1e6:.0f} MB out > 126 MB L2); no explicit flush",
                        "grid": {"dims": dims, "bits": bits}, "edge_capacity": cap, "parallelism": f"events sharded over {rank.world_size} GPU(s), no collective"},
-            "edges_per_event": e_mean, "roofline": roofline, "path_roofline": path_roofline, "phases_us": phases_us,
+            "edges_per_event": e_mean, "roofline": roofline, "path_roofline": path_roofline, "phases_us": phases_us, "timeline_us": timeline_us,
             "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
             "gpu_launches_per_step": launches_per_step, "clocks": clocks,
             "host_wall_ms_per_step": 1e3 * (t1 - t0) / args.steps,

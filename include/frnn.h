@@ -21,7 +21,8 @@
  *   - Every pointer is a DEVICE pointer owned by the caller unless marked HOST.  The library never
  *     allocates or frees caller-visible memory.  frnn_build_ex / frnn_build_batched only enqueue
  *     work on `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and never synchronise.
- *   - points: row-major n x dim fp32, base 16-byte aligned, finite values (non-finite coordinates
+ *   - points: row-major n x dim fp32, base 32-byte aligned (a row moves as one 256-bit transaction;
+ *     FRNN_ERR_INVALID_ARG otherwise), finite values (non-finite coordinates
  *     are a precondition violation; they can never cause an out-of-bounds access).
  *   - src/dst are int32 row indices (local to the event in the batched call); counts and offsets
  *     are int64.  Edges of one call are sorted by (src, dst) ascending and free of duplicates.
@@ -47,7 +48,7 @@ extern "C" {
 
 typedef enum {
     FRNN_OK = 0,
-    FRNN_ERR_INVALID_ARG = -1,  /* null pointer, n < 0, r < 0 or not finite, k_max < 1, bad offsets */
+    FRNN_ERR_INVALID_ARG = -1,  /* null or misaligned pointer, n < 0, r < 0 or not finite, k_max < 1, bad offsets */
     FRNN_ERR_UNSUPPORTED = -2,  /* dim != 8, more than 2^31-1 rows */
     FRNN_ERR_CAPACITY = -3,     /* device-detected: more edges than edge_capacity */
     FRNN_ERR_WORKSPACE = -4,    /* workspace_bytes < frnn_workspace_bytes(...) */
@@ -150,6 +151,19 @@ int frnn_last_launch_count(void);
 int frnn_set_profiling(int enabled);
 int frnn_get_profile(float* phase_ms /* HOST */, int max_phases);
 const char* frnn_phase_name(int phase);
+
+/*
+ * In-graph timeline.  frnn_set_profiling(2) (instead of 1) keeps the CUDA-graph replay and makes every
+ * kernel of later calls leave the earliest start and the latest end of its warps (%globaltimer) in the
+ * call's workspace; frnn_get_timeline synchronises nothing itself (the caller waits for the call first),
+ * copies the stamps of the LAST call that used `workspace` (a device pointer; n_total / n_events as in
+ * that call) and writes, per kernel (bin, scan_cells, scatter, search, emit), begin and end in
+ * microseconds relative to the start of the first kernel.  Returns the number of kernels written or a
+ * negative status.  Unlike mode 1 this does not perturb the launch sequence.
+ */
+int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events,
+                      double* begin_us /* HOST */, double* end_us /* HOST */, int max_phases);
+const char* frnn_timeline_name(int phase);
 
 /* Release the cached workspace / staging buffers of frnn_build and frnn_build_host. */
 void frnn_release_cached(void);

@@ -20,6 +20,9 @@ constexpr size_t kAlign = 256;
 
 int g_force_dims = 0, g_force_bits = 0;
 int g_use_graph = 1;
+bool g_timeline = false;                    // frnn_set_profiling(2): kernels leave %globaltimer stamps in the workspace
+constexpr int kTimelinePhases = 5;
+const char* const kTimelineNames[kTimelinePhases] = {"bin", "scan_cells", "scatter", "search", "emit"};
 thread_local int t_launches = 0;
 
 // Optional per-phase CUDA-event timing (frnn_set_profiling): one event after every phase.
@@ -59,7 +62,7 @@ struct Layout {
     int rows_per_block;
     int64_t scan_blocks;
     size_t off_cells, off_tiles, off_counters, zero_bytes;
-    size_t off_pcell, off_prank, off_spts, off_sidx, off_scell, off_skey, off_cnt, off_evoff, off_hits;
+    size_t off_pcell, off_prank, off_spts, off_sidx, off_skey, off_cnt, off_evoff, off_hits;
     size_t total;
 };
 
@@ -76,7 +79,7 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     size_t o = 0;
     L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_entries + 8) * 4);
     L.off_tiles = o;    o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8 * kDegSlices);
-    L.off_counters = o; o = align_up(o + 64);          // [0..3] cursor of the cell scan (u32)
+    L.off_counters = o; o = align_up(o + 256);         // [0..3] cursor of the cell scan (u32); [64..) timeline stamps (u64 x 2 x kTimelinePhases)
     const size_t n = static_cast<size_t>(n_total > 0 ? n_total : 1);
     L.off_cnt = o;      o = align_up(o + n * 4);       // zeroed: the search pass counts with atomics
     L.zero_bytes = o;
@@ -84,7 +87,6 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     L.off_prank = o;  o = align_up(o + n * 4);
     L.off_spts = o;   o = align_up(o + n * 32);
     L.off_sidx = o;   o = align_up(o + n * 4);
-    L.off_scell = o;  o = align_up(o + n * 4);
     L.off_skey = o;   o = align_up(o + n * 4);
     L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
     L.off_hits = o;   o = align_up(o + n * kSlot * sizeof(int2));
@@ -109,6 +111,7 @@ int check_common(const float* points, int64_t n, int dim, float r, int k_max, co
     if (n < 0 || k_max < 1 || capacity < 0) return FRNN_ERR_INVALID_ARG;
     if (!(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
     if (n > 0 && !points) return FRNN_ERR_INVALID_ARG;
+    if (reinterpret_cast<uintptr_t>(points) % 32) return FRNN_ERR_INVALID_ARG;      // rows move as 256-bit transactions
     if (capacity > 0 && (!out_src || !out_dst || !out_d2)) return FRNN_ERR_INVALID_ARG;
     if (dim != kDim) return FRNN_ERR_UNSUPPORTED;
     if (n > 0x7fffffffll) return FRNN_ERR_UNSUPPORTED;
@@ -131,11 +134,12 @@ struct Call {                 // everything that determines the enqueued work (a
     void* workspace;
     int grid_dims, grid_bits;
     std::vector<int64_t> ev_off;
+    bool timeline = false;
     bool operator==(const Call& o) const {
         return points == o.points && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
                out_dst == o.out_dst && out_d2 == o.out_d2 && capacity == o.capacity && out_count == o.out_count &&
                out_edge_offsets == o.out_edge_offsets && out_status == o.out_status && out_row_ptr == o.out_row_ptr &&
-               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off;
+               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline;
     }
 };
 
@@ -146,11 +150,11 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
     unsigned long long* tile_deg = reinterpret_cast<unsigned long long*>(ws + L.off_tiles);
     unsigned int* cursor = reinterpret_cast<unsigned int*>(ws + L.off_counters);
+    unsigned long long* stamps = c.timeline ? reinterpret_cast<unsigned long long*>(ws + L.off_counters + 64) : nullptr;
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
     int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
-    uint32_t* scell = reinterpret_cast<uint32_t*>(ws + L.off_scell);
     uint32_t* skey = reinterpret_cast<uint32_t*>(ws + L.off_skey);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
     int64_t* ev_off = reinterpret_cast<int64_t*>(ws + L.off_evoff);
@@ -180,19 +184,20 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     }
     mark(0, st);
     const unsigned row_blocks = static_cast<unsigned>((n_total + 255) / 256);
-    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank)));
+    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(1, st);
-    cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor);
+    cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor, stamps);
     ++t_launches; CK(cudaGetLastError());
     mark(2, st);
-    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, scell, skey)));
+    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(3, st);
 
     SearchArgs sa;
-    sa.spts = spts; sa.sidx = sidx; sa.scell = scell; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
-    sa.tile_deg = tile_deg; sa.n_total = n_total; sa.r2 = r2; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
+    sa.spts = spts; sa.sidx = sidx; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
+    sa.tile_deg = tile_deg; sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
+    sa.inv_cell = inv_cell; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
     const unsigned search_blocks = static_cast<unsigned>((n_total + kSearchThreads - 1) / kSearchThreads);
     FRNN_DISPATCH_G(G, (search_kernel<GG><<<search_blocks, kSearchThreads, 0, st>>>(sa)));
     ++t_launches; CK(cudaGetLastError());
@@ -203,7 +208,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     ea.tile_deg = tile_deg; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
-    ea.k_max = static_cast<uint32_t>(c.k_max);
+    ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps;
     FRNN_DISPATCH_G(G, (emit_kernel<GG><<<static_cast<unsigned>(L.emit_tiles), kEmitThreads, 0, st>>>(ea)));
     ++t_launches; CK(cudaGetLastError());
     mark(5, st);
@@ -275,6 +280,7 @@ int prepare(Call& c, size_t workspace_bytes) {
     const GridChoice g = choose_grid(n_total, c.n_events);
     c.grid_dims = g.dims;
     c.grid_bits = g.bits;
+    c.timeline = g_timeline;
     if (n_total == 0) return FRNN_OK;
     const Layout L = make_layout(n_total, c.n_events, g);
     if (!c.workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
@@ -309,7 +315,7 @@ int ensure_stream() {
 
 extern "C" {
 
-int frnn_version(void) { return 200; }   // 0.2.0
+int frnn_version(void) { return 300; }   // 0.3.0
 
 const char* frnn_status_string(int status) {
     switch (status) {
@@ -437,6 +443,8 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
 int frnn_last_launch_count(void) { return t_launches; }
 
 int frnn_set_profiling(int enabled) {
+    g_timeline = enabled == 2;
+    if (enabled == 2) enabled = 0;
     if (enabled && !g_ev_valid) {
         for (int i = 0; i <= kPhases; ++i)
             if (cudaEventCreate(&g_ev[i]) != cudaSuccess) return FRNN_ERR_CUDA;
@@ -454,6 +462,23 @@ int frnn_get_profile(float* phase_ms, int max_phases) {
         if (cudaEventElapsedTime(&phase_ms[i], g_ev[i], g_ev[i + 1]) != cudaSuccess) return FRNN_ERR_CUDA;
     return n;
 }
+
+int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, double* begin_us, double* end_us, int max_phases) {
+    if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1) return FRNN_ERR_INVALID_ARG;
+    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events));
+    unsigned long long h[2 * kTimelinePhases];
+    if (cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess)
+        return FRNN_ERR_CUDA;
+    const int n = max_phases < kTimelinePhases ? max_phases : kTimelinePhases;
+    const unsigned long long t0 = ~h[0];                   // start of the first kernel
+    for (int i = 0; i < n; ++i) {
+        begin_us[i] = 1e-3 * static_cast<double>(static_cast<long long>(~h[2 * i] - t0));
+        end_us[i] = 1e-3 * static_cast<double>(static_cast<long long>(h[2 * i + 1] - t0));
+    }
+    return n;
+}
+
+const char* frnn_timeline_name(int phase) { return (phase >= 0 && phase < kTimelinePhases) ? kTimelineNames[phase] : ""; }
 
 const char* frnn_phase_name(int phase) { return (phase >= 0 && phase < kPhases) ? kPhaseNames[phase] : ""; }
 

@@ -89,6 +89,33 @@ __device__ __forceinline__ float d2_pinned(const float4& qa, const float4& qb, c
     return acc;
 }
 
+// One 32-byte row = one 256-bit transaction (LDG.E.ENL2.256 / STG.E.ENL2.256 on sm_100a).  The .nc form is
+// only used on arrays that no thread writes during the kernel.
+__device__ __forceinline__ void load_row_nc(const float4* p, float4& a, float4& b) {
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(p));
+}
+__device__ __forceinline__ void store_row(float4* p, const float4& a, const float4& b) {
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w) : "memory");
+}
+
+// Optional in-graph timeline (frnn_set_profiling(2)): every kernel leaves min(start) and max(end) of its
+// warps' %globaltimer readings in stamps[2*phase], stamps[2*phase+1] (start stored complemented so that
+// one atomicMax serves both; the buffer is zeroed with the rest of the workspace head).  stamps == NULL
+// (the normal case) costs one predictable branch per warp.
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void stamp_begin(unsigned long long* stamps, int phase) {
+    if (stamps && (threadIdx.x & 31) == 0) atomicMax(&stamps[2 * phase], ~global_ns());
+}
+__device__ __forceinline__ void stamp_end(unsigned long long* stamps, int phase) {
+    if (stamps && (threadIdx.x & 31) == 0) atomicMax(&stamps[2 * phase + 1], global_ns());
+}
+
 __device__ __forceinline__ int event_of_row(const int64_t* __restrict__ ev_off, int n_events, int64_t row) {
     int lo = 0, hi = n_events;                 // largest e with ev_off[e] <= row
     while (hi - lo > 1) {
@@ -117,16 +144,20 @@ __global__ void __launch_bounds__(256) bin_kernel(const float4* __restrict__ pts
                                                   const int64_t* __restrict__ ev_off, int n_events,
                                                   float inv_cell, int bits,
                                                   uint32_t* __restrict__ cell_count,
-                                                  uint32_t* __restrict__ pcell, uint32_t* __restrict__ prank) {
+                                                  uint32_t* __restrict__ pcell, uint32_t* __restrict__ prank,
+                                                  unsigned long long* stamps) {
+    stamp_begin(stamps, 0);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n_total) return;
-    const float4 a = pts[2 * i];
-    float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (G > 4) b = pts[2 * i + 1];
-    const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
-    const uint32_t lin = cell_of_point<G>(a, b, ev, inv_cell, bits);
-    pcell[i] = lin;
-    prank[i] = atomicAdd(&cell_count[padded(lin, bits)], 1u);
+    if (i < n_total) {
+        const float4 a = pts[2 * i];
+        float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (G > 4) b = pts[2 * i + 1];
+        const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
+        const uint32_t lin = cell_of_point<G>(a, b, ev, inv_cell, bits);
+        pcell[i] = lin;
+        prank[i] = atomicAdd(&cell_count[padded(lin, bits)], 1u);
+    }
+    stamp_end(stamps, 0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -139,17 +170,18 @@ __global__ void __launch_bounds__(256) scatter_kernel(const float4* __restrict__
                                                       const uint32_t* __restrict__ pcell,
                                                       const uint32_t* __restrict__ prank,
                                                       float4* __restrict__ spts, int32_t* __restrict__ sidx,
-                                                      uint32_t* __restrict__ scell, uint32_t* __restrict__ skey) {
+                                                      uint32_t* __restrict__ skey, unsigned long long* stamps) {
+    stamp_begin(stamps, 2);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i >= n_total) return;
-    const uint32_t lin = pcell[i];
-    const uint32_t s = cell_start[padded(lin, bits)] + prank[i];
-    const float4 a = pts[2 * i], b = pts[2 * i + 1];
-    spts[2 * static_cast<int64_t>(s)] = a;
-    spts[2 * static_cast<int64_t>(s) + 1] = b;
-    sidx[s] = static_cast<int32_t>(i);
-    scell[s] = lin;
-    skey[s] = key_of_point<G>(a, b, inv_cell);
+    if (i < n_total) {
+        const uint32_t s = cell_start[padded(pcell[i], bits)] + prank[i];
+        float4 a, b;
+        load_row_nc(pts + 2 * i, a, b);
+        store_row(spts + 2 * static_cast<int64_t>(s), a, b);      // one 32-byte sector, one transaction
+        sidx[s] = static_cast<int32_t>(i);
+        skey[s] = key_of_point<G>(a, b, inv_cell);
+    }
+    stamp_end(stamps, 2);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -165,7 +197,9 @@ constexpr int kCellTile = 4 * kCellThreads;      // table entries per block (upp
 // A block owns `rows_per_block` whole padded rows = rows_per_block * (2^bits + 1) <= kCellTile
 // entries (a multiple of 4, so every thread moves one aligned uint4).
 __global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __restrict__ cells, int64_t n_entries, int rows_per_block,
-                                                                 int bits, unsigned int* __restrict__ cursor) {
+                                                                 int bits, unsigned int* __restrict__ cursor,
+                                                                 unsigned long long* stamps) {
+    stamp_begin(stamps, 1);
     __shared__ uint32_t s_pts[32];
     __shared__ uint32_t s_base;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -197,11 +231,13 @@ __global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __res
         if (lane == 31) s_base = sp ? atomicAdd(cursor, sp) : 0u;
     }
     __syncthreads();
-    if (!act) return;
-    const uint32_t p = s_base + s_pts[warp] + (ip - tp);
-    uint4 out;
-    out.x = p; out.y = p + v.x; out.z = out.y + v.y; out.w = out.z + v.z;
-    *reinterpret_cast<uint4*>(cells + blk_base + local) = out;
+    if (act) {
+        const uint32_t p = s_base + s_pts[warp] + (ip - tp);
+        uint4 out;
+        out.x = p; out.y = p + v.x; out.z = out.y + v.y; out.w = out.z + v.z;
+        *reinterpret_cast<uint4*>(cells + blk_base + local) = out;
+    }
+    stamp_end(stamps, 1);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -340,19 +376,21 @@ constexpr int kBatch = 4;              // candidates of a run tested per batch
 constexpr int kQueue = 32;             // survivor queue entries per thread (>= 2 * 3 * kBatch)
 constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
 constexpr int kEmitThreads = 512;      // rows per emit tile
-constexpr int kDegSlices = 32;         // copies of every per-tile degree counter (spreads same-address atomics)
+constexpr int kDegSlices = 4;          // copies of every per-tile degree counter (spreads same-address atomics)
 
 struct SearchArgs {
     const float4* spts;
     const int32_t* sidx;          // slot -> global row index
-    const uint32_t* scell;        // slot -> linear cell id
     const uint32_t* skey;         // slot -> filter key
     const uint32_t* cell_start;
     uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index (zeroed)
     int2* hits;                   // [n_total * kSlot] (j global, d2 bits)
     unsigned long long* tile_deg; // [ceil(n_total / kEmitThreads) * kDegSlices] partial sums of min(|S_i|, k_max) per emit tile (zeroed)
+    const int64_t* ev_off;        // device event offsets or NULL for one event
+    unsigned long long* stamps;   // NULL unless the timeline is being recorded
     int64_t n_total;
-    float r2;
+    int n_events;
+    float r2, inv_cell;
     int bits;
     uint32_t k_max;
 };
@@ -363,36 +401,58 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     constexpr int NB = pow3(G >= 2 ? G - 2 : 0);          // sub-batches: offsets of coordinates 0..G-3 (dim 0 most significant)
     constexpr int MID = (NB - 1) / 2;                     // the sub-batch with all-zero offsets
     __shared__ uint32_t s_queue[kQueue + 1][kSearchThreads];
+    stamp_begin(a.stamps, 3);
     const int tid = threadIdx.x;
     const int64_t s64 = static_cast<int64_t>(blockIdx.x) * kSearchThreads + tid;
-    if (s64 >= a.n_total) return;                         // no block-wide barrier below
+    if (s64 >= a.n_total) { stamp_end(a.stamps, 3); return; }      // no block-wide barrier below
     const uint32_t s = static_cast<uint32_t>(s64);
-    const float4 qa = a.spts[2 * s64], qb = a.spts[2 * s64 + 1];
+    float4 qa, qb;
+    load_row_nc(a.spts + 2 * s64, qa, qb);
     const int32_t my_row = a.sidx[s];
-    const uint32_t cell = a.scell[s];
     const uint32_t key_a = a.skey[s] + kKeyBias;
     const int bits = a.bits;
     const uint32_t mask = (1u << bits) - 1u;
+    // the slot's cell, recomputed from its coordinates (the event from the row index: blocks of the cell-ordered
+    // copy land in arrival order, so slots are not ordered by event)
+    const uint32_t ev = a.ev_off ? static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, my_row)) : 0u;
+    const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, bits);
     const uint32_t c_last = cell & mask;
     const uint32_t lo = c_last ? c_last - 1u : 0u, hi = c_last < mask ? c_last + 1u : mask;
-    const bool seam = c_last == 0u || c_last == mask;
-    const uint32_t wrap_cell = c_last == 0u ? mask : 0u;
     const uint32_t deg_slice = blockIdx.x & (kDegSlices - 1);
+    // interior in the coordinates 0..G-2: a neighbour row is the own row plus a constant (no wrap)
+    bool interior = true;
+#pragma unroll
+    for (int d = 0; d < G - 1; ++d) {
+        const uint32_t cd = (cell >> ((G - 1 - d) * bits)) & mask;
+        interior = interior && cd != 0u && cd != mask;
+    }
+    const uint32_t own_rowid = cell >> bits;
     uint32_t own_deg = 0;                                 // increments of cnt[my_row] made here that found a value < k_max
     uint32_t* qp = &s_queue[0][tid];                      // next free queue entry
     uint32_t* const q0 = qp;
     constexpr int kQStride = kSearchThreads;              // in words
 
+    // A hit (i, j, d2): pos = cnt[i]++ and hits[i * kSlot + pos] = (j, d2) if pos < kSlot, the same for j.  The
+    // two returning atomics are issued at the hit, their results are consumed ("retired") only at the NEXT hit
+    // or at the end of the thread, so the L2 round trip overlaps the evaluation of the following candidates.
+    int32_t pend_j = -1, pend_d2 = 0;
+    uint32_t pend_p = 0, pend_q = 0;
+    auto retire = [&]() {
+        if (pend_j >= 0) {
+            if (pend_p < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + pend_p] = make_int2(pend_j, pend_d2);
+            if (pend_q < kSlot) a.hits[static_cast<int64_t>(pend_j) * kSlot + pend_q] = make_int2(my_row, pend_d2);
+            own_deg += pend_p < a.k_max;
+            if (pend_q < a.k_max) atomicAdd(&a.tile_deg[(pend_j / kEmitThreads) * kDegSlices + deg_slice], 1ull);
+        }
+    };
     auto test = [&](const float4& ca, const float4& cb, int32_t cj) {
         const float d2 = d2_pinned(qa, qb, ca, cb);
         if (d2 <= a.r2) {
-            const int d2b = __float_as_int(d2);
-            const uint32_t p = atomicAdd(&a.cnt[my_row], 1u);
-            const uint32_t q = atomicAdd(&a.cnt[cj], 1u);
-            if (p < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + p] = make_int2(cj, d2b);
-            if (q < kSlot) a.hits[static_cast<int64_t>(cj) * kSlot + q] = make_int2(my_row, d2b);
-            own_deg += p < a.k_max;
-            if (q < a.k_max) atomicAdd(&a.tile_deg[(cj / kEmitThreads) * kDegSlices + deg_slice], 1ull);
+            retire();
+            pend_p = atomicAdd(&a.cnt[my_row], 1u);
+            pend_q = atomicAdd(&a.cnt[cj], 1u);
+            pend_j = cj;
+            pend_d2 = __float_as_int(d2);
         }
     };
     // phase 2: evaluate the queued survivors (never the query itself)
@@ -401,16 +461,16 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
         qp = q0;
         if (qn == 0) return;
         uint32_t j = q0[0];
-        float4 xa = a.spts[2 * static_cast<int64_t>(j)], xb = a.spts[2 * static_cast<int64_t>(j) + 1];
+        float4 xa, xb, ya, yb;
+        load_row_nc(a.spts + 2 * static_cast<int64_t>(j), xa, xb);
         int32_t xj = a.sidx[j];
-        float4 ya, yb;
         int32_t yj;
         int i = 1;
         while (true) {
-            if (i < qn) { j = q0[i * kQStride]; ya = a.spts[2 * static_cast<int64_t>(j)]; yb = a.spts[2 * static_cast<int64_t>(j) + 1]; yj = a.sidx[j]; }
+            if (i < qn) { j = q0[i * kQStride]; load_row_nc(a.spts + 2 * static_cast<int64_t>(j), ya, yb); yj = a.sidx[j]; }
             test(xa, xb, xj);
             if (++i > qn) break;
-            if (i < qn) { j = q0[i * kQStride]; xa = a.spts[2 * static_cast<int64_t>(j)]; xb = a.spts[2 * static_cast<int64_t>(j) + 1]; xj = a.sidx[j]; }
+            if (i < qn) { j = q0[i * kQStride]; load_row_nc(a.spts + 2 * static_cast<int64_t>(j), xa, xb); xj = a.sidx[j]; }
             test(ya, yb, yj);
             if (++i > qn) break;
         }
@@ -422,8 +482,24 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
         *qp = j;
         qp += pass ? kQStride : 0;
     };
-    // padded table index of cell 0 of the neighbour row: coordinates 0..G-3 offset by the base-3 digits
-    // of b (coordinate 0 most significant), coordinate G-2 by u - 1 (wrapped)
+    // a run of candidate slots [j0, j1), kBatch keys in flight
+    auto scan_run = [&](uint32_t j0, uint32_t j1) {
+        for (; j0 < j1; j0 += kBatch) {
+            if (qp - q0 > (kQueue - kBatch) * kQStride) drain();
+            const uint32_t* kp = a.skey + j0;
+            const uint32_t len = j1 - j0;
+            uint32_t kr[kBatch];
+#pragma unroll
+            for (int v = 0; v < kBatch; ++v) {
+                kr[v] = 0u;
+                if (static_cast<uint32_t>(v) < len) kr[v] = kp[v];
+            }
+#pragma unroll
+            for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, j0 + v, kr[v]);
+        }
+    };
+    // general form: padded table index of cell 0 of the neighbour row with coordinates 0..G-3 offset by the
+    // base-3 digits of b (coordinate 0 most significant) and coordinate G-2 by u - 1, all wrapped
     auto row_of = [&](int b, int u) -> uint32_t {
         uint32_t base = cell >> (G * bits);               // event index
 #pragma unroll
@@ -438,13 +514,27 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
 
     for (int b = MID; b < NB; ++b) {
         const bool zero = b == MID;                       // row offsets 0 in coordinates 0..G-3
+        uint32_t row[NU];
+        if (interior) {
+            int delta = 0, bb = b;                        // neighbour row id - own row id for u = 1
+#pragma unroll
+            for (int d = G - 3; d >= 0; --d) { delta += (bb % 3 - 1) * (1 << ((G - 2 - d) * bits)); bb /= 3; }
+            const uint32_t mid_row = own_rowid + static_cast<uint32_t>(delta);
+#pragma unroll
+            for (int u = 0; u < NU; ++u) {
+                const uint32_t rid = mid_row + static_cast<uint32_t>((G >= 2 ? u : 1) - 1);
+                row[u] = (rid << bits) + rid;
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < NU; ++u) row[u] = row_of(b, G >= 2 ? u : 1);
+        }
         uint32_t rs[NU], re[NU];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
             const int uu = G >= 2 ? u : 1;
-            const uint32_t row = row_of(b, uu);
-            rs[u] = a.cell_start[row + lo];
-            re[u] = a.cell_start[row + hi + 1u];
+            rs[u] = a.cell_start[row[u] + lo];
+            re[u] = a.cell_start[row[u] + hi + 1u];
             if (zero && uu == 1) rs[u] = s + 1u;          // own row: the slots after mine (my cell and the next one)
             if (zero && uu == 0) re[u] = rs[u];           // backward row: its queries come to me
         }
@@ -466,40 +556,33 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
 #pragma unroll
             for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, rs[u] + v, kc[u][v]);
         }
-        // runs longer than kBatch, and the wrapped cell of lanes on the seam of the torus: batches of
-        // kBatch in ONE copy of the loop (the run is picked with selects so rs/re stay in registers)
-        for (int t = 0; t < (seam ? 2 * NU : NU); ++t) {
-            const int u = t < NU ? t : t - NU;
+        // runs longer than kBatch: ONE copy of the loop (the run is picked with selects so rs/re stay in registers)
+        for (int t = 0; t < NU; ++t) {
             uint32_t j0 = rs[0] + kBatch, j1 = re[0];
 #pragma unroll
             for (int w = 1; w < NU; ++w)
-                if (u == w) { j0 = rs[w] + kBatch; j1 = re[w]; }
-            if (t >= NU) {
-                const int uu = G >= 2 ? u : 1;
-                const uint32_t row = row_of(b, uu);
-                j0 = a.cell_start[row + wrap_cell];
-                j1 = a.cell_start[row + wrap_cell + 1u];
-                // own row: only the cell after mine is forward; backward row: nothing
-                if (zero && (uu == 0 || (uu == 1 && c_last != mask))) j1 = j0;
-            }
-            for (; j0 < j1; j0 += kBatch) {
-                if (qp - q0 > (kQueue - kBatch) * kQStride) drain();
-                const uint32_t* kp = a.skey + j0;
-                const uint32_t len = j1 - j0;
-                uint32_t kr[kBatch];
-#pragma unroll
-                for (int v = 0; v < kBatch; ++v) {
-                    kr[v] = 0u;
-                    if (static_cast<uint32_t>(v) < len) kr[v] = kp[v];
-                }
-#pragma unroll
-                for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, j0 + v, kr[v]);
-            }
+                if (t == w) { j0 = rs[w] + kBatch; j1 = re[w]; }
+            scan_run(j0, j1);
         }
     }
+    // Slots whose cell touches the seam of the torus in the last coordinate (only points beyond +-2^(bits-1)
+    // cells from the origin) also visit the wrapped cell of every forward row: cold code.
+    if (c_last == 0u || c_last == mask) {
+        const uint32_t wrap_cell = c_last == 0u ? mask : 0u;
+        for (int b = MID; b < NB; ++b)
+            for (int u = 0; u < NU; ++u) {
+                const int uu = G >= 2 ? u : 1;
+                // own row: only the cell after mine is forward; backward row: nothing
+                if (b == MID && (uu == 0 || (uu == 1 && c_last != mask))) continue;
+                const uint32_t r = row_of(b, uu);
+                scan_run(a.cell_start[r + wrap_cell], a.cell_start[r + wrap_cell + 1u]);
+            }
+    }
     drain();
+    retire();
     // per-tile degree totals: emit_kernel turns them into its global offsets without any inter-block wait
     if (own_deg) atomicAdd(&a.tile_deg[(my_row / kEmitThreads) * kDegSlices + deg_slice], static_cast<unsigned long long>(own_deg));
+    stamp_end(a.stamps, 3);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -562,6 +645,7 @@ struct EmitArgs {
     int64_t* out_count;           // optional
     int64_t* out_edge_offsets;    // optional [n_events + 1]
     int32_t* out_status;
+    unsigned long long* stamps;   // NULL unless the timeline is being recorded
     float r2, inv_cell;
     int bits;
     uint32_t k_max;
@@ -633,21 +717,21 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
 
 template <int G>
 __global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
+    __shared__ unsigned long long s_rp[kEmitThreads + 1];  // offsets of the tile's rows inside the tile (capped degrees)
     __shared__ unsigned long long s_warp[kEmitThreads / 32];
     __shared__ unsigned long long s_prefix;
+    __shared__ int32_t s_evb[kEmitThreads];                // first row of the event of every row (batched calls)
+    __shared__ uint32_t s_bigmask[kEmitThreads / 32];
     __shared__ int s_delta[kEmitThreads / 32][32];
+    stamp_begin(a.stamps, 4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t tile = blockIdx.x;
-    const int64_t i = static_cast<int64_t>(tile) * kEmitThreads + threadIdx.x;
+    const int64_t tile_row0 = static_cast<int64_t>(tile) * kEmitThreads;
+    const int64_t i = tile_row0 + threadIdx.x;
     const bool has = i < a.n_total;
     const uint32_t c = has ? a.cnt[i] : 0u;
     const uint32_t deg = c < a.k_max ? c : a.k_max;
-    // first hits of the row: issued early so the loads overlap the offset computation
-    const int2* h = a.hits + i * kSlot;
-    int4 h01 = make_int4(0, 0, 0, 0), h23 = h01;
-    if (c > 0) h01 = *reinterpret_cast<const int4*>(h);
-    if (c > 2) h23 = *reinterpret_cast<const int4*>(h + 2);
     // ---- global offset of the tile = sum of the totals of the tiles before it
     unsigned long long before = 0;
     for (uint32_t t = threadIdx.x; t < tile * kDegSlices; t += kEmitThreads) before += a.tile_deg[t];
@@ -669,12 +753,19 @@ __global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
         if (lane == 0) s_prefix = b;
     }
     __syncthreads();
-    if (lane == 31) s_warp[warp] = incl;                   // warp totals of deg (fits: <= 32 * k_max... use 64-bit)
+    if (lane == 31) s_warp[warp] = incl;                   // warp totals of deg
     __syncthreads();
     unsigned long long wexcl = 0;
 #pragma unroll
     for (int w = 0; w < kEmitThreads / 32; ++w) wexcl += (w < warp) ? s_warp[w] : 0ull;
-    const int64_t rp = static_cast<int64_t>(s_prefix + wexcl + (incl - deg));      // row_ptr[i]
+    const unsigned long long local_rp = wexcl + (incl - deg);
+    const unsigned long long tile_base = s_prefix;
+    const int64_t rp = static_cast<int64_t>(tile_base + local_rp);                 // row_ptr[i]
+    const bool big = has && (c > kSlot || c > a.k_max);
+    s_rp[threadIdx.x] = local_rp;
+    if (threadIdx.x == kEmitThreads - 1) s_rp[kEmitThreads] = local_rp + deg;
+    const uint32_t bigs_warp = __ballot_sync(kFull, big);
+    if (lane == 0) s_bigmask[warp] = bigs_warp;
     // ---- CSR offsets, count, status, per-event edge offsets
     int64_t ev_base = 0;
     if (has) {
@@ -694,54 +785,63 @@ __global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
             *a.out_status = total > a.capacity ? -3 /* FRNN_ERR_CAPACITY */ : 0;
         }
     }
-    // ---- rows that fit their slot buffer: rank by dst, place directly
-    const bool big = has && (c > kSlot || c > a.k_max);
-    if (has && !big && c > 0) {
-        const int32_t src = static_cast<int32_t>(i - ev_base);
-        const int32_t eb = static_cast<int32_t>(ev_base);
-        auto put = [&](uint32_t rank, int32_t j, int32_t d2bits) {
-            const int64_t pos = rp + rank;
-            if (pos < a.capacity) { a.out_src[pos] = src; a.out_dst[pos] = j - eb; a.out_d2[pos] = __int_as_float(d2bits); }
-        };
-        if (c <= 4) {                                      // the common case: everything is already in registers
-            const int32_t j0 = h01.x, j1 = c > 1 ? h01.z : 0x7fffffff, j2 = c > 2 ? h23.x : 0x7fffffff, j3 = c > 3 ? h23.z : 0x7fffffff;
-            put((j1 < j0) + (j2 < j0) + (j3 < j0), j0, h01.y);
-            if (c > 1) put((j0 < j1) + (j2 < j1) + (j3 < j1), j1, h01.w);
-            if (c > 2) put((j0 < j2) + (j1 < j2) + (j3 < j2), j2, h23.y);
-            if (c > 3) put((j0 < j3) + (j1 < j3) + (j2 < j3), j3, h23.w);
-        } else {
-            for (uint32_t m = 0; m < c; ++m) {
-                const int2 mine = h[m];
-                uint32_t rank = 0;
-                for (uint32_t u = 0; u < c; ++u) rank += h[u].x < mine.x;
-                put(rank, mine.x, mine.y);
-            }
+    s_evb[threadIdx.x] = static_cast<int32_t>(ev_base);
+    __syncthreads();
+    // ---- rows that fit their slot buffer, ONE THREAD PER OUTPUT EDGE: edge p of the tile belongs to the row r
+    // with s_rp[r] <= p < s_rp[r+1] (binary search in shared memory), is the row's hit number m = p - s_rp[r],
+    // and goes to position rank(dst among the row's hits): no sort, coalesced work, the COO comes out sorted.
+    const unsigned long long tile_edges = s_rp[kEmitThreads];
+    for (unsigned long long p = threadIdx.x; p < tile_edges; p += kEmitThreads) {
+        int r = 0;
+#pragma unroll
+        for (int step = kEmitThreads / 2; step >= 1; step >>= 1)
+            if (s_rp[r + step] <= p) r += step;
+        if ((s_bigmask[r >> 5] >> (r & 31)) & 1u) continue;            // resolved below by a whole warp
+        const unsigned long long r0 = s_rp[r];
+        const uint32_t cr = static_cast<uint32_t>(s_rp[r + 1] - r0);   // = uncapped count (the row is not big)
+        const uint32_t m = static_cast<uint32_t>(p - r0);
+        const int64_t row = tile_row0 + r;
+        const int2* h = a.hits + row * kSlot;
+        const int2 mine = h[m];
+        uint32_t rank = 0;
+        for (uint32_t u = 0; u < cr; u += 2) {                         // two hits per 16-byte load (slot buffers are padded)
+            const int4 v = *reinterpret_cast<const int4*>(h + u);
+            rank += (v.x < mine.x) + (u + 1 < cr && v.z < mine.x);
+        }
+        const int64_t pos = static_cast<int64_t>(tile_base + r0) + rank;
+        if (pos < a.capacity) {
+            const int32_t eb = s_evb[r];
+            a.out_src[pos] = static_cast<int32_t>(row) - eb;
+            a.out_dst[pos] = mine.x - eb;
+            a.out_d2[pos] = __int_as_float(mine.y);
         }
     }
     // ---- big rows: recompute with the whole warp
-    uint32_t bigs = __ballot_sync(kFull, big);
-    if (bigs == 0) return;
-    int lane_delta = lane_row_delta<G>(lane, a.bits);
-    const uint32_t mask = (1u << a.bits) - 1u;
-    for (; bigs; bigs &= bigs - 1) {
-        const int bl = __ffs(bigs) - 1;
-        const int64_t row = __shfl_sync(kFull, i, bl);
-        const int64_t row_rp = __shfl_sync(kFull, rp, bl);
-        const int64_t row_ev = __shfl_sync(kFull, ev_base, bl);
-        const uint32_t row_cnt = __shfl_sync(kFull, c, bl);
-        const float4 qa = a.pts[2 * row], qb = a.pts[2 * row + 1];
-        uint32_t ev = 0;
-        if (a.ev_off) ev = static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, row));
-        const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, a.bits);
-        bool interior = true;
+    uint32_t bigs = bigs_warp;
+    if (bigs != 0) {
+        int lane_delta = lane_row_delta<G>(lane, a.bits);
+        const uint32_t mask = (1u << a.bits) - 1u;
+        for (; bigs; bigs &= bigs - 1) {
+            const int bl = __ffs(bigs) - 1;
+            const int64_t row = __shfl_sync(kFull, i, bl);
+            const int64_t row_rp = __shfl_sync(kFull, rp, bl);
+            const int64_t row_ev = __shfl_sync(kFull, ev_base, bl);
+            const uint32_t row_cnt = __shfl_sync(kFull, c, bl);
+            const float4 qa = a.pts[2 * row], qb = a.pts[2 * row + 1];
+            uint32_t ev = 0;
+            if (a.ev_off) ev = static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, row));
+            const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, a.bits);
+            bool interior = true;
 #pragma unroll
-        for (int d = 0; d < G; ++d) {
-            const uint32_t cd = (cell >> (d * a.bits)) & mask;
-            interior = interior && cd != 0u && cd != mask;
+            for (int d = 0; d < G; ++d) {
+                const uint32_t cd = (cell >> (d * a.bits)) & mask;
+                interior = interior && cd != 0u && cd != mask;
+            }
+            if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
+            else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
         }
-        if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
-        else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
     }
+    stamp_end(a.stamps, 4);
 }
 
 }  // namespace frnn

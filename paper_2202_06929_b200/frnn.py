@@ -45,6 +45,8 @@ _SIGNATURES = {
     "frnn_set_profiling": (_c.c_int, [_c.c_int]),
     "frnn_get_profile": (_c.c_int, [_c.POINTER(_c.c_float), _c.c_int]),
     "frnn_phase_name": (_c.c_char_p, [_c.c_int]),
+    "frnn_get_timeline": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_double), _c.c_int]),
+    "frnn_timeline_name": (_c.c_char_p, [_c.c_int]),
     "frnn_release_cached": (None, []),
 }
 EXPORTED_SYMBOLS = tuple(_SIGNATURES)
@@ -112,8 +114,19 @@ def frnn_last_launch_count() -> int:
     return lib().frnn_last_launch_count()
 
 
-def frnn_set_profiling(enabled: bool) -> None:
-    _check(lib().frnn_set_profiling(int(bool(enabled))), "frnn_set_profiling")
+def frnn_set_profiling(enabled) -> None:
+    """0/False: off; 1/True: one CUDA event after every phase; 2: in-graph %globaltimer timeline."""
+    _check(lib().frnn_set_profiling(int(enabled)), "frnn_set_profiling")
+
+
+def frnn_get_timeline(workspace: torch.Tensor, n_total: int, n_events: int = 1) -> dict[str, tuple[float, float]]:
+    """(begin_us, end_us) per kernel of the last call on ``workspace`` made in profiling mode 2
+    (the caller synchronises first)."""
+    b, e = (_c.c_double * 8)(), (_c.c_double * 8)()
+    n = lib().frnn_get_timeline(_ptr(workspace), int(n_total), int(n_events), b, e, 8)
+    if n < 0:
+        raise FrnnError(n, "frnn_get_timeline")
+    return {lib().frnn_timeline_name(i).decode(): (float(b[i]), float(e[i])) for i in range(n)}
 
 
 def frnn_get_profile() -> dict[str, float]:

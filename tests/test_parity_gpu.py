@@ -216,6 +216,7 @@ def test_host_detectable_errors(F):
     assert call(**args(r=float("inf"))) == F.FRNN_ERR_INVALID_ARG
     assert call(**args(k=0)) == F.FRNN_ERR_INVALID_ARG
     assert call(**args(p=None)) == F.FRNN_ERR_INVALID_ARG
+    assert call(**args(p=pts.data_ptr() + 16)) == F.FRNN_ERR_INVALID_ARG      # rows must be 32-byte aligned
     assert call(**args(dim=3)) == F.FRNN_ERR_UNSUPPORTED
     assert call(**args(), wsbytes=128) == F.FRNN_ERR_WORKSPACE
     torch.cuda.synchronize()
@@ -265,3 +266,28 @@ def test_repeated_calls_reuse_workspace_and_are_deterministic(F):
     for o in outs[1:]:
         assert all(np.array_equal(a, b) for a, b in zip(o, outs[0]))
     assert F.frnn_last_launch_count() >= 6
+
+
+def test_timeline_mode_gives_the_same_result_and_ordered_stamps(F):
+    """Profiling mode 2: kernels stamp %globaltimer into the workspace; results are unchanged."""
+    cfg = events.CONFIGS[1]
+    x = events.make_event(cfg)
+    exp = oracle.frnn(x, cfg.r, cfg.k_max, oracle.CELLS)
+    pts = torch.from_numpy(x).cuda()
+    ws = F.Workspace(cfg.n, 1, cfg.k_max, cfg.n * 8)
+    st = torch.cuda.Stream()
+    try:
+        F.frnn_set_profiling(2)
+        res = F.frnn_build_ex(pts, cfg.r, cfg.k_max, ws=ws, stream=st)
+        st.synchronize()
+        tl = F.frnn_get_timeline(ws.buf, cfg.n, 1)
+    finally:
+        F.frnn_set_profiling(0)
+    s, d, q = (t.cpu().numpy() for t in res.trimmed())
+    assert_same(Got(s, d, q), exp, cfg.r, "timeline mode")
+    names = list(tl)
+    assert names == ["bin", "scan_cells", "scatter", "search", "emit"]
+    assert tl["bin"][0] == 0.0
+    for a, b in zip(names, names[1:]):
+        assert tl[a][0] <= tl[a][1] <= tl[b][0] + 1e-9, (a, b, tl)        # kernels of one call are serialised
+    assert tl["emit"][1] < 1e5                                            # microseconds, not garbage
