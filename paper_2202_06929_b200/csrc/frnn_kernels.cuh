@@ -100,8 +100,8 @@ __device__ __forceinline__ void store_row(float4* p, const float4& a, const floa
                  :: "l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w) : "memory");
 }
 
-// Optional in-graph timeline (frnn_set_profiling(2)): every kernel leaves min(start) and max(end) of its
-// warps' %globaltimer readings in stamps[2*phase], stamps[2*phase+1] (start stored complemented so that
+// Optional in-graph timeline (frnn_set_profiling(2)): every kernel leaves min(start) and max(end) of the
+// %globaltimer readings of thread 0 of its blocks (every 16th block for the start) in stamps[2*phase], stamps[2*phase+1] (start stored complemented so that
 // one atomicMax serves both; the buffer is zeroed with the rest of the workspace head).  stamps == NULL
 // (the normal case) costs one predictable branch per warp.
 __device__ __forceinline__ unsigned long long global_ns() {
@@ -110,10 +110,10 @@ __device__ __forceinline__ unsigned long long global_ns() {
     return t;
 }
 __device__ __forceinline__ void stamp_begin(unsigned long long* stamps, int phase) {
-    if (stamps && (threadIdx.x & 31) == 0) atomicMax(&stamps[2 * phase], ~global_ns());
+    if (stamps && threadIdx.x == 0 && (blockIdx.x & 15) == 0) atomicMax(&stamps[2 * phase], ~global_ns());
 }
 __device__ __forceinline__ void stamp_end(unsigned long long* stamps, int phase) {
-    if (stamps && (threadIdx.x & 31) == 0) atomicMax(&stamps[2 * phase + 1], global_ns());
+    if (stamps && threadIdx.x == 0) atomicMax(&stamps[2 * phase + 1], global_ns());
 }
 
 __device__ __forceinline__ int event_of_row(const int64_t* __restrict__ ev_off, int n_events, int64_t row) {
@@ -395,12 +395,29 @@ struct SearchArgs {
     uint32_t k_max;
 };
 
+// Filter test + push of one candidate slot j: if the key passes, j is stored at the thread's queue address
+// and the address advances by one entry -- four SASS instructions (IADD, LOP3 to a predicate, predicated
+// STS and IADD), no branch, no 64-bit pointer arithmetic.
+__device__ __forceinline__ void filter_push(uint32_t& qaddr, uint32_t key_a, uint32_t key_c, uint32_t j) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .u32 t;\n\t"
+        "sub.u32 t, %1, %2;\n\t"
+        "and.b32 t, t, %4;\n\t"
+        "setp.eq.u32 p, t, 0;\n\t"
+        "@p st.shared.u32 [%0], %3;\n\t"
+        "@p add.u32 %0, %0, %5;\n\t}"
+        : "+r"(qaddr)
+        : "r"(key_a), "r"(key_c), "r"(j), "n"(kKeyReject), "n"(kSearchThreads * 4)
+        : "memory");
+}
+
 template <int G>
 __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search_kernel(SearchArgs a) {
     constexpr int NU = G >= 2 ? 3 : 1;                    // unrolled offsets of coordinate G-2
     constexpr int NB = pow3(G >= 2 ? G - 2 : 0);          // sub-batches: offsets of coordinates 0..G-3 (dim 0 most significant)
     constexpr int MID = (NB - 1) / 2;                     // the sub-batch with all-zero offsets
-    __shared__ uint32_t s_queue[kQueue + 1][kSearchThreads];
+    constexpr int kWide = 4;                              // survivors evaluated together (rows in flight per thread)
+    __shared__ uint32_t s_queue[kQueue][kSearchThreads];
     stamp_begin(a.stamps, 3);
     const int tid = threadIdx.x;
     const int64_t s64 = static_cast<int64_t>(blockIdx.x) * kSearchThreads + tid;
@@ -410,6 +427,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     load_row_nc(a.spts + 2 * s64, qa, qb);
     const int32_t my_row = a.sidx[s];
     const uint32_t key_a = a.skey[s] + kKeyBias;
+    const uint32_t key_fail = key_a - 4u;                 // a candidate key that never passes: (key_a - key_fail) & reject = 4
     const int bits = a.bits;
     const uint32_t mask = (1u << bits) - 1u;
     // the slot's cell, recomputed from its coordinates (the event from the row index: blocks of the cell-ordered
@@ -428,74 +446,70 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     }
     const uint32_t own_rowid = cell >> bits;
     uint32_t own_deg = 0;                                 // increments of cnt[my_row] made here that found a value < k_max
-    uint32_t* qp = &s_queue[0][tid];                      // next free queue entry
-    uint32_t* const q0 = qp;
-    constexpr int kQStride = kSearchThreads;              // in words
+    const uint32_t q_base = static_cast<uint32_t>(__cvta_generic_to_shared(&s_queue[0][tid]));
+    uint32_t qaddr = q_base;                              // shared-memory address of the next free queue entry
+    constexpr uint32_t kQBytes = kSearchThreads * 4;      // one queue entry further down the thread's column
 
-    // A hit (i, j, d2): pos = cnt[i]++ and hits[i * kSlot + pos] = (j, d2) if pos < kSlot, the same for j.  The
-    // two returning atomics are issued at the hit, their results are consumed ("retired") only at the NEXT hit
-    // or at the end of the thread, so the L2 round trip overlaps the evaluation of the following candidates.
-    int32_t pend_j = -1, pend_d2 = 0;
-    uint32_t pend_p = 0, pend_q = 0;
-    auto retire = [&]() {
-        if (pend_j >= 0) {
-            if (pend_p < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + pend_p] = make_int2(pend_j, pend_d2);
-            if (pend_q < kSlot) a.hits[static_cast<int64_t>(pend_j) * kSlot + pend_q] = make_int2(my_row, pend_d2);
-            own_deg += pend_p < a.k_max;
-            if (pend_q < a.k_max) atomicAdd(&a.tile_deg[(pend_j / kEmitThreads) * kDegSlices + deg_slice], 1ull);
-        }
-    };
-    auto test = [&](const float4& ca, const float4& cb, int32_t cj) {
-        const float d2 = d2_pinned(qa, qb, ca, cb);
-        if (d2 <= a.r2) {
-            retire();
-            pend_p = atomicAdd(&a.cnt[my_row], 1u);
-            pend_q = atomicAdd(&a.cnt[cj], 1u);
-            pend_j = cj;
-            pend_d2 = __float_as_int(d2);
-        }
-    };
-    // phase 2: evaluate the queued survivors (never the query itself)
+    // phase 2: evaluate the queued survivors (never the query itself), kWide at a time: kWide 256-bit row
+    // loads in flight, then the R3 chains, then -- for the hits (i, j, d2) -- ONE returning atomic on cnt[i]
+    // for all hits of the group and one per partner row j, all in flight together, then the stores
+    // hits[row * kSlot + pos] = (other, d2) for pos < kSlot on both rows.  The counts keep running beyond kSlot,
+    // which tells emit_kernel to resolve that row by recomputation; min(cnt, k_max) is the number of increments
+    // that found a value < k_max, so the per-tile capped degree totals are accumulated by the same increments.
     auto drain = [&]() {
-        const int qn = static_cast<int>(qp - q0) / kQStride;
-        qp = q0;
-        if (qn == 0) return;
-        uint32_t j = q0[0];
-        float4 xa, xb, ya, yb;
-        load_row_nc(a.spts + 2 * static_cast<int64_t>(j), xa, xb);
-        int32_t xj = a.sidx[j];
-        int32_t yj;
-        int i = 1;
-        while (true) {
-            if (i < qn) { j = q0[i * kQStride]; load_row_nc(a.spts + 2 * static_cast<int64_t>(j), ya, yb); yj = a.sidx[j]; }
-            test(xa, xb, xj);
-            if (++i > qn) break;
-            if (i < qn) { j = q0[i * kQStride]; load_row_nc(a.spts + 2 * static_cast<int64_t>(j), xa, xb); xj = a.sidx[j]; }
-            test(ya, yb, yj);
-            if (++i > qn) break;
+        const int qn = static_cast<int>((qaddr - q_base) / kQBytes);
+        qaddr = q_base;
+        for (int i = 0; i < qn; i += kWide) {
+            float4 ca[kWide], cb[kWide];
+            int32_t cj[kWide];
+            bool ok[kWide];
+#pragma unroll
+            for (int v = 0; v < kWide; ++v) {
+                ok[v] = i + v < qn;
+                const uint32_t j = ok[v] ? s_queue[i + v][tid] : s;      // padding: my own row (a valid address, masked below)
+                load_row_nc(a.spts + 2 * static_cast<int64_t>(j), ca[v], cb[v]);
+                cj[v] = a.sidx[j];
+            }
+            float d2[kWide];
+            uint32_t nh = 0;
+#pragma unroll
+            for (int v = 0; v < kWide; ++v) {
+                d2[v] = d2_pinned(qa, qb, ca[v], cb[v]);
+                ok[v] = ok[v] && d2[v] <= a.r2;
+                nh += ok[v];
+            }
+            if (nh == 0) continue;
+            uint32_t pos = atomicAdd(&a.cnt[my_row], nh);
+            uint32_t pq[kWide];
+#pragma unroll
+            for (int v = 0; v < kWide; ++v)
+                if (ok[v]) pq[v] = atomicAdd(&a.cnt[cj[v]], 1u);
+#pragma unroll
+            for (int v = 0; v < kWide; ++v)
+                if (ok[v]) {
+                    const int d2b = __float_as_int(d2[v]);
+                    if (pos < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + pos] = make_int2(cj[v], d2b);
+                    if (pq[v] < kSlot) a.hits[static_cast<int64_t>(cj[v]) * kSlot + pq[v]] = make_int2(my_row, d2b);
+                    own_deg += pos < a.k_max;
+                    if (pq[v] < a.k_max) atomicAdd(&a.tile_deg[(cj[v] / kEmitThreads) * kDegSlices + deg_slice], 1ull);
+                    ++pos;
+                }
         }
-    };
-    // phase 1 for one candidate slot: branch-free push (the entry is only kept if the pointer advances);
-    // the caller guarantees one free entry
-    auto filter = [&](bool valid, uint32_t j, uint32_t key_c) {
-        const bool pass = valid && ((key_a - key_c) & kKeyReject) == 0u;
-        *qp = j;
-        qp += pass ? kQStride : 0;
     };
     // a run of candidate slots [j0, j1), kBatch keys in flight
     auto scan_run = [&](uint32_t j0, uint32_t j1) {
         for (; j0 < j1; j0 += kBatch) {
-            if (qp - q0 > (kQueue - kBatch) * kQStride) drain();
+            if (qaddr - q_base > (kQueue - kBatch) * kQBytes) drain();
             const uint32_t* kp = a.skey + j0;
             const uint32_t len = j1 - j0;
             uint32_t kr[kBatch];
 #pragma unroll
             for (int v = 0; v < kBatch; ++v) {
-                kr[v] = 0u;
+                kr[v] = key_fail;
                 if (static_cast<uint32_t>(v) < len) kr[v] = kp[v];
             }
 #pragma unroll
-            for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, j0 + v, kr[v]);
+            for (int v = 0; v < kBatch; ++v) filter_push(qaddr, key_a, kr[v], j0 + v);
         }
     };
     // general form: padded table index of cell 0 of the neighbour row with coordinates 0..G-3 offset by the
@@ -538,7 +552,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
             if (zero && uu == 1) rs[u] = s + 1u;          // own row: the slots after mine (my cell and the next one)
             if (zero && uu == 0) re[u] = rs[u];           // backward row: its queries come to me
         }
-        if (qp - q0 > (kQueue - NU * kBatch) * kQStride) drain();
+        if (qaddr - q_base > (kQueue - NU * kBatch) * kQBytes) drain();
         uint32_t kc[NU][kBatch];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
@@ -546,16 +560,14 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
             const uint32_t len = re[u] - rs[u];
 #pragma unroll
             for (int v = 0; v < kBatch; ++v) {
-                kc[u][v] = 0u;
+                kc[u][v] = key_fail;
                 if (static_cast<uint32_t>(v) < len) kc[u][v] = kp[v];
             }
         }
 #pragma unroll
-        for (int u = 0; u < NU; ++u) {
-            const uint32_t len = re[u] - rs[u];
+        for (int u = 0; u < NU; ++u)
 #pragma unroll
-            for (int v = 0; v < kBatch; ++v) filter(static_cast<uint32_t>(v) < len, rs[u] + v, kc[u][v]);
-        }
+            for (int v = 0; v < kBatch; ++v) filter_push(qaddr, key_a, kc[u][v], rs[u] + v);
         // runs longer than kBatch: ONE copy of the loop (the run is picked with selects so rs/re stay in registers)
         for (int t = 0; t < NU; ++t) {
             uint32_t j0 = rs[0] + kBatch, j1 = re[0];
@@ -579,7 +591,6 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
             }
     }
     drain();
-    retire();
     // per-tile degree totals: emit_kernel turns them into its global offsets without any inter-block wait
     if (own_deg) atomicAdd(&a.tile_deg[(my_row / kEmitThreads) * kDegSlices + deg_slice], static_cast<unsigned long long>(own_deg));
     stamp_end(a.stamps, 3);
