@@ -196,7 +196,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
 
     SearchArgs sa;
     sa.spts = spts; sa.sidx = sidx; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
-    sa.tile_deg = tile_deg; sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
+    sa.tile_deg = tile_deg; sa.n_tiles = static_cast<uint32_t>(L.emit_tiles); sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
     sa.inv_cell = inv_cell; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
     const unsigned search_blocks = static_cast<unsigned>((n_total + kSearchThreads - 1) / kSearchThreads);
     FRNN_DISPATCH_G(G, (search_kernel<GG><<<search_blocks, kSearchThreads, 0, st>>>(sa)));

@@ -372,11 +372,20 @@ constexpr int kSearchThreads = 128;
 #ifndef FRNN_SEARCH_MIN_BLOCKS
 #define FRNN_SEARCH_MIN_BLOCKS 7       // 7 x 128 threads: 72 registers per thread; 7 x 148 blocks >= one 120k-point event
 #endif
-constexpr int kBatch = 4;              // candidates of a run tested per batch
+#ifndef FRNN_KBATCH
+#define FRNN_KBATCH 3
+#endif
+constexpr int kBatch = FRNN_KBATCH;    // candidates of a run tested per batch
 constexpr int kQueue = 32;             // survivor queue entries per thread (>= 2 * 3 * kBatch)
 constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
-constexpr int kEmitThreads = 512;      // rows per emit tile
-constexpr int kDegSlices = 4;          // copies of every per-tile degree counter (spreads same-address atomics)
+#ifndef FRNN_EMIT_THREADS
+#define FRNN_EMIT_THREADS 256
+#endif
+constexpr int kEmitThreads = FRNN_EMIT_THREADS;   // rows per emit tile
+#ifndef FRNN_DEG_SLICES
+#define FRNN_DEG_SLICES 8
+#endif
+constexpr int kDegSlices = FRNN_DEG_SLICES;   // copies of every per-tile degree counter, slice-major: the copies of a tile sit in different sectors
 
 struct SearchArgs {
     const float4* spts;
@@ -385,7 +394,8 @@ struct SearchArgs {
     const uint32_t* cell_start;
     uint32_t* cnt;                // [n_total] uncapped |S_i| at the global row index (zeroed)
     int2* hits;                   // [n_total * kSlot] (j global, d2 bits)
-    unsigned long long* tile_deg; // [ceil(n_total / kEmitThreads) * kDegSlices] partial sums of min(|S_i|, k_max) per emit tile (zeroed)
+    unsigned long long* tile_deg; // [kDegSlices][n_tiles] partial sums of min(|S_i|, k_max) per emit tile (zeroed)
+    uint32_t n_tiles;             // ceil(n_total / kEmitThreads)
     const int64_t* ev_off;        // device event offsets or NULL for one event
     unsigned long long* stamps;   // NULL unless the timeline is being recorded
     int64_t n_total;
@@ -436,7 +446,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, bits);
     const uint32_t c_last = cell & mask;
     const uint32_t lo = c_last ? c_last - 1u : 0u, hi = c_last < mask ? c_last + 1u : mask;
-    const uint32_t deg_slice = blockIdx.x & (kDegSlices - 1);
+    unsigned long long* const my_tile_deg = a.tile_deg + static_cast<size_t>(blockIdx.x & (kDegSlices - 1)) * a.n_tiles;
     // interior in the coordinates 0..G-2: a neighbour row is the own row plus a constant (no wrap)
     bool interior = true;
 #pragma unroll
@@ -491,7 +501,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
                     if (pos < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + pos] = make_int2(cj[v], d2b);
                     if (pq[v] < kSlot) a.hits[static_cast<int64_t>(cj[v]) * kSlot + pq[v]] = make_int2(my_row, d2b);
                     own_deg += pos < a.k_max;
-                    if (pq[v] < a.k_max) atomicAdd(&a.tile_deg[(cj[v] / kEmitThreads) * kDegSlices + deg_slice], 1ull);
+                    if (pq[v] < a.k_max) atomicAdd(&my_tile_deg[cj[v] / kEmitThreads], 1ull);
                     ++pos;
                 }
         }
@@ -592,7 +602,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     }
     drain();
     // per-tile degree totals: emit_kernel turns them into its global offsets without any inter-block wait
-    if (own_deg) atomicAdd(&a.tile_deg[(my_row / kEmitThreads) * kDegSlices + deg_slice], static_cast<unsigned long long>(own_deg));
+    if (own_deg) atomicAdd(&my_tile_deg[my_row / kEmitThreads], static_cast<unsigned long long>(own_deg));
     stamp_end(a.stamps, 3);
 }
 
@@ -727,7 +737,7 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
 }
 
 template <int G>
-__global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
+__global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel(EmitArgs a) {
     __shared__ unsigned long long s_rp[kEmitThreads + 1];  // offsets of the tile's rows inside the tile (capped degrees)
     __shared__ unsigned long long s_warp[kEmitThreads / 32];
     __shared__ unsigned long long s_prefix;
@@ -745,7 +755,13 @@ __global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
     const uint32_t deg = c < a.k_max ? c : a.k_max;
     // ---- global offset of the tile = sum of the totals of the tiles before it
     unsigned long long before = 0;
-    for (uint32_t t = threadIdx.x; t < tile * kDegSlices; t += kEmitThreads) before += a.tile_deg[t];
+    for (uint32_t t = threadIdx.x; t < tile; t += kEmitThreads) {
+        unsigned long long part[kDegSlices];
+#pragma unroll
+        for (int sl = 0; sl < kDegSlices; ++sl) part[sl] = a.tile_deg[static_cast<size_t>(sl) * gridDim.x + t];      // all in flight
+#pragma unroll
+        for (int sl = 0; sl < kDegSlices; ++sl) before += part[sl];
+    }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) before += __shfl_xor_sync(kFull, before, o);
     // ---- block scan of deg
@@ -760,7 +776,7 @@ __global__ void __launch_bounds__(kEmitThreads, 2) emit_kernel(EmitArgs a) {
     if (warp == 0) {
         unsigned long long b = lane < kEmitThreads / 32 ? s_warp[lane] : 0ull;
 #pragma unroll
-        for (int o = 8; o >= 1; o >>= 1) b += __shfl_xor_sync(kFull, b, o);
+        for (int o = 16; o >= 1; o >>= 1) b += __shfl_xor_sync(kFull, b, o);
         if (lane == 0) s_prefix = b;
     }
     __syncthreads();
