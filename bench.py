@@ -180,7 +180,7 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--pool", type=int, default=POOL)
-    ap.add_argument("--cpu-events", type=int, default=24, help="events the cpu_baseline leg runs the oracle on")
+    ap.add_argument("--cpu-events", type=int, default=160, help="events the cpu_baseline leg runs the oracle on")
     ap.add_argument("--e2e-steps", type=int, default=1000)
     ap.add_argument("--profile-steps", type=int, default=200)
     ap.add_argument("--timeline-steps", type=int, default=100)
