@@ -165,6 +165,39 @@ int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events,
                       double* begin_us /* HOST */, double* end_us /* HOST */, int max_phases);
 const char* frnn_timeline_name(int phase);
 
+/*
+ * ---- The two steps that consume the edge list ----
+ *
+ * frnn_gather_edge_rows -- input rows of the edge-filtering stage.  PAPER.md:31 (section 2): the filter is a
+ * classifier on EDGES, i.e. on the features of both end points; PAPER.md:37 (section 3): it is fed "in batches of
+ * 800,000 edges".  For every edge e in [e_begin, min(e_begin + e_max, *edge_count)):
+ *     out[(e - e_begin) * 2*dim + 0 .. dim)      = points[(src[e] + row_base) * dim ..]
+ *     out[(e - e_begin) * 2*dim + dim .. 2*dim)  = points[(dst[e] + row_base) * dim ..]
+ * All pointers are DEVICE pointers.  points: n x dim fp32 (dim == 8), 32-byte aligned; out: room for e_max rows of
+ * 2*dim floats, 32-byte aligned; edge_count: device int64 (the out_count of frnn_build_ex) or NULL (then exactly
+ * e_max edges are gathered); row_base: added to src/dst (event_offsets[e] for the local indices of a batched
+ * build, else 0).  src/dst + row_base must lie in [0, n) (precondition; indices are clamped, never read out of
+ * bounds).  Asynchronous on cuda_stream.  Returns FRNN_OK or a negative status; nothing is enqueued on error.
+ */
+int frnn_gather_edge_rows(const float* points, int64_t n, int dim, const int32_t* src, const int32_t* dst,
+                          const int64_t* edge_count, int64_t e_begin, int64_t e_max, int64_t row_base,
+                          float* out, void* cuda_stream);
+
+/*
+ * frnn_label_components -- track labelling.  PAPER.md:33 (section 2): edges whose score passes a threshold are
+ * kept and the connected components of what remains are the track candidates; PAPER.md:61 (section 3.2): weakly
+ * connected components on the GPU.  Over the nodes 0..n-1 and the edges e < min(edge_max, *edge_count) with
+ * score[e] >= threshold (score == NULL: every edge), direction ignored:
+ *     labels[i] = the smallest node index in the component of node i   (canonical: one correct answer)
+ *     *n_components = number of components (isolated nodes count)      (optional, may be NULL)
+ * All pointers are DEVICE pointers (labels int32[n], n_components int32[1], edge_count int64[1] or NULL).
+ * Edges with an end point outside [0, n) and self loops are ignored.  No workspace: labels doubles as the
+ * union-find parent array.  Asynchronous on cuda_stream.  Returns FRNN_OK or a negative status.
+ */
+int frnn_label_components(int64_t n, const int32_t* src, const int32_t* dst, const float* score, float threshold,
+                          const int64_t* edge_count, int64_t edge_max, int32_t* labels, int32_t* n_components,
+                          void* cuda_stream);
+
 /* Release the cached workspace / staging buffers of frnn_build and frnn_build_host. */
 void frnn_release_cached(void);
 

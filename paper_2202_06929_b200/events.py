@@ -110,3 +110,16 @@ def uniform_points(n: int, dim: int, lo: float, hi: float, seed: int) -> np.ndar
 def shard_events(n_events: int, world_size: int, rank: int) -> list[int]:
     """Round-robin event -> rank assignment (events are independent units)."""
     return list(range(rank, n_events, world_size))
+
+
+def edge_scores(n_edges: int, seed: int) -> np.ndarray:
+    """Stand-in for the GNN's per-edge scores (the trained GNN is not available): seeded U[0,1) fp32."""
+    rng = np.random.default_rng(seed)
+    return np.ascontiguousarray(rng.random(n_edges, dtype=np.float32))
+
+
+def random_graph(n: int, n_edges: int, seed: int):
+    """Seeded random directed edge list (src, dst int32) with possible self loops and duplicates."""
+    rng = np.random.default_rng(seed)
+    return (np.ascontiguousarray(rng.integers(0, n, n_edges, dtype=np.int32)),
+            np.ascontiguousarray(rng.integers(0, n, n_edges, dtype=np.int32)))

@@ -47,6 +47,10 @@ _SIGNATURES = {
     "frnn_phase_name": (_c.c_char_p, [_c.c_int]),
     "frnn_get_timeline": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_double), _c.c_int]),
     "frnn_timeline_name": (_c.c_char_p, [_c.c_int]),
+    "frnn_gather_edge_rows": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p,
+                                         _c.c_int64, _c.c_int64, _c.c_int64, _c.c_void_p, _c.c_void_p]),
+    "frnn_label_components": (_c.c_int, [_c.c_int64, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_float, _c.c_void_p,
+                                         _c.c_int64, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
     "frnn_release_cached": (None, []),
 }
 EXPORTED_SYMBOLS = tuple(_SIGNATURES)
@@ -264,3 +268,41 @@ def frnn_build_host(points_host: torch.Tensor, r: float, k_max: int, out_src: to
                                cap, _c.byref(count))
     _check(st, "frnn_build_host")
     return count.value
+
+
+def frnn_gather_edge_rows(points: torch.Tensor, src: torch.Tensor, dst: torch.Tensor, edge_count: torch.Tensor | None = None,
+                          e_begin: int = 0, e_max: int | None = None, row_base: int = 0, out: torch.Tensor | None = None,
+                          stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+    """[x_src || x_dst] rows of the edges [e_begin, min(e_begin + e_max, edge_count)) (the filter stage's input)."""
+    _require_cuda(points)
+    n, dim = points.shape
+    if e_max is None:
+        e_max = src.numel() - e_begin
+    if out is None:
+        out = torch.empty((max(e_max, 0), 2 * dim), dtype=torch.float32, device=points.device)
+    stream = stream or torch.cuda.current_stream(points.device)
+    st = lib().frnn_gather_edge_rows(_ptr(points), n, dim, _ptr(src), _ptr(dst), _ptr(edge_count), int(e_begin), int(e_max),
+                                     int(row_base), _ptr(out), _c.c_void_p(stream.cuda_stream))
+    _check(st, "frnn_gather_edge_rows")
+    return out
+
+
+def frnn_label_components(n: int, src: torch.Tensor, dst: torch.Tensor, score: torch.Tensor | None = None, threshold: float = 0.0,
+                          edge_count: torch.Tensor | None = None, edge_max: int | None = None,
+                          labels: torch.Tensor | None = None, n_components: torch.Tensor | None = None,
+                          stream: torch.cuda.Stream | None = None):
+    """labels[i] = smallest node index of the weakly connected component of i; returns (labels, n_components)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2202_06929_b200 needs a CUDA device (no CPU fallback)")
+    dev = src.device
+    if edge_max is None:
+        edge_max = src.numel()
+    if labels is None:
+        labels = torch.empty(max(n, 1), dtype=torch.int32, device=dev)[:n]
+    if n_components is None:
+        n_components = torch.zeros(1, dtype=torch.int32, device=dev)
+    stream = stream or torch.cuda.current_stream(dev)
+    st = lib().frnn_label_components(int(n), _ptr(src), _ptr(dst), _ptr(score), float(threshold), _ptr(edge_count), int(edge_max),
+                                     _ptr(labels), _ptr(n_components), _c.c_void_p(stream.cuda_stream))
+    _check(st, "frnn_label_components")
+    return labels, n_components
