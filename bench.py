@@ -184,6 +184,7 @@ def main() -> None:
     ap.add_argument("--e2e-steps", type=int, default=1000)
     ap.add_argument("--profile-steps", type=int, default=200)
     ap.add_argument("--timeline-steps", type=int, default=100)
+    ap.add_argument("--next-steps", type=int, default=300, help="timed repetitions of the two edge-list consumers (0: skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -325,6 +326,47 @@ def main() -> None:
                      "compulsory_dram_bytes": n * 32.0 + 12.0 * e_mean,
                      "compulsory_frac": (n * 32.0 + 12.0 * e_mean) / t_event / 1e9 / peak}
 
+    # the two steps that consume the edge list, timed on the outputs of the pool
+    next_rows = None
+    if args.next_steps > 0:
+        e_cap = max(edges_per_event)
+        rows_out = [torch.empty((e_cap, 16), dtype=torch.float32, device=dev) for _ in range(4)]      # 4 x 21.5 MB
+        labels = torch.empty(n, dtype=torch.int32, device=dev)
+        ncomp = torch.zeros(1, dtype=torch.int32, device=dev)
+        scores = torch.from_numpy(events.edge_scores(e_cap, 1)).to(dev)
+
+        def t_loop(fn, reps):
+            with torch.cuda.stream(stream):
+                for i in range(5):
+                    fn(i)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for i in range(reps):
+                    fn(i)
+                b.record(stream)
+                stream.synchronize()
+            return 1e3 * a.elapsed_time(b) / reps
+
+        def gather(i):
+            k = i % len(outs)
+            F.frnn_gather_edge_rows(pts[k], outs[k].src, outs[k].dst, edge_count=outs[k].count, e_max=e_cap,
+                                    out=rows_out[i % 4], stream=stream)
+
+        def label(i):
+            k = i % len(outs)
+            F.frnn_label_components(n, outs[k].src, outs[k].dst, score=scores, threshold=0.5, edge_count=outs[k].count,
+                                    edge_max=e_cap, labels=labels, n_components=ncomp, stream=stream)
+
+        g_us, l_us = t_loop(gather, args.next_steps), t_loop(label, args.next_steps)
+        g_bytes = e_mean * (8 + 64 + 64)
+        next_rows = {
+            "gather_edge_rows": {"us_per_event": g_us, "edges": e_mean, "algorithmic_bytes": g_bytes,
+                                 "achieved_gbs": g_bytes / (g_us * 1e-6) / 1e9, "frac_of_hbm_peak": g_bytes / (g_us * 1e-6) / 1e9 / peak,
+                                 "note": "per edge: 8 B indices + 2 x 32 B rows read (L2) + 64 B written (streaming stores)"},
+            "label_components": {"us_per_event": l_us, "nodes": n, "edges": e_mean, "threshold": 0.5,
+                                 "components": int(ncomp.item()), "note": "3 kernels: init, hook (CAS union-find), flatten"},
+        }
+
     # end to end through the host-buffer entry point: pinned host buffers, copies inside the timed region
     e2e = None
     if args.e2e_steps > 0:
@@ -366,7 +408,7 @@ def main() -> None:
                              f"{len(seeds) * cap * 12 / 1e6:.0f} MB out > 126 MB L2); no explicit flush",
                        "grid": {"dims": dims, "bits": bits}, "edge_capacity": cap, "parallelism": f"events sharded over {rank.world_size} GPU(s), no collective"},
             "edges_per_event": e_mean, "roofline": roofline, "path_roofline": path_roofline, "phases_us": phases_us, "timeline_us": timeline_us,
-            "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+            "cpu_baseline": cpu_baseline, "e2e": e2e, "next_rows": next_rows, "gpu_launches": launches_per_step * args.steps,
             "gpu_launches_per_step": launches_per_step, "clocks": clocks,
             "host_wall_ms_per_step": 1e3 * (t1 - t0) / args.steps,
             "paper_context": "paper: 0.04 +- 0.01 s/event on V100 16 GB (PAPER.md:77 Table 1 'FRNN' column), TrackML events; other machine, other data",

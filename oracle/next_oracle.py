@@ -12,7 +12,7 @@ label_components   PAPER.md:33 (section 2: edges whose score passes a threshold 
                    be reached from i over kept edges, direction ignored.  Computed as the fixed point of
                    "every node takes the minimum label among itself and its neighbours", which is that
                    definition iterated (at most diameter + 1 sweeps).
-Readings (DESIGN.md section 12): an edge is kept when score >= threshold (inclusive); self loops and edges with
+Readings (DESIGN.md section 11): an edge is kept when score >= threshold (inclusive); self loops and edges with
 an end point outside [0, n) are ignored; isolated nodes are components of their own.
 """
 from __future__ import annotations
