@@ -51,6 +51,11 @@ _SIGNATURES = {
                                          _c.c_int64, _c.c_int64, _c.c_int64, _c.c_void_p, _c.c_void_p]),
     "frnn_label_components": (_c.c_int, [_c.c_int64, _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_float, _c.c_void_p,
                                          _c.c_int64, _c.c_void_p, _c.c_void_p, _c.c_void_p]),
+    "frnn_host_pipeline_create": (_c.c_int, [_c.c_int64, _c.c_int, _c.c_int, _c.c_int64, _c.c_int, _c.POINTER(_c.c_void_p)]),
+    "frnn_host_pipeline_submit": (_c.c_int, [_c.c_void_p, _c.c_void_p, _c.c_int64, _c.c_float, _c.c_void_p, _c.c_void_p,
+                                             _c.c_void_p, _c.c_void_p]),
+    "frnn_host_pipeline_wait": (_c.c_int, [_c.c_void_p]),
+    "frnn_host_pipeline_destroy": (None, [_c.c_void_p]),
     "frnn_release_cached": (None, []),
 }
 EXPORTED_SYMBOLS = tuple(_SIGNATURES)
@@ -306,3 +311,34 @@ def frnn_label_components(n: int, src: torch.Tensor, dst: torch.Tensor, score: t
                                      _ptr(labels), _ptr(n_components), _c.c_void_p(stream.cuda_stream))
     _check(st, "frnn_label_components")
     return labels, n_components
+
+
+class HostPipeline:
+    """frnn_host_pipeline_*: a stream of host-resident events with copies and builds overlapped."""
+
+    def __init__(self, n_max: int, k_max: int, edge_capacity: int, depth: int = 3):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2202_06929_b200 needs a CUDA device (no CPU fallback)")
+        self._h = _c.c_void_p()
+        _check(lib().frnn_host_pipeline_create(int(n_max), 8, int(k_max), int(edge_capacity), int(depth), _c.byref(self._h)),
+               "frnn_host_pipeline_create")
+
+    def submit(self, points_host: torch.Tensor, r: float, out_src: torch.Tensor, out_dst: torch.Tensor, out_d2: torch.Tensor,
+               out_count: torch.Tensor) -> None:
+        n = points_host.shape[0]
+        _check(lib().frnn_host_pipeline_submit(self._h, _ptr(points_host), n, float(r), _ptr(out_src), _ptr(out_dst), _ptr(out_d2),
+                                               _ptr(out_count)), "frnn_host_pipeline_submit")
+
+    def wait(self) -> None:
+        _check(lib().frnn_host_pipeline_wait(self._h), "frnn_host_pipeline_wait")
+
+    def close(self) -> None:
+        if self._h:
+            lib().frnn_host_pipeline_destroy(self._h)
+            self._h = _c.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

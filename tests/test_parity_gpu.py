@@ -291,3 +291,31 @@ def test_timeline_mode_gives_the_same_result_and_ordered_stamps(F):
     for a, b in zip(names, names[1:]):
         assert tl[a][0] <= tl[a][1] <= tl[b][0] + 1e-9, (a, b, tl)        # kernels of one call are serialised
     assert tl["emit"][1] < 1e5                                            # microseconds, not garbage
+
+
+def test_host_pipeline_overlapped_events(F):
+    """frnn_host_pipeline_*: seven events through three slots, results in pinned host buffers, count on the host."""
+    cfg = events.CONFIGS[0]
+    cap = cfg.n * 8
+    pipe = F.HostPipeline(cfg.n, cfg.k_max, cap, depth=3)
+    xs = [events.make_event(cfg, 20 + i)[: cfg.n - 37 * i] for i in range(7)]
+    pins = [torch.from_numpy(x).pin_memory() for x in xs]
+    outs = [(torch.empty(cap, dtype=torch.int32).pin_memory(), torch.empty(cap, dtype=torch.int32).pin_memory(),
+             torch.empty(cap, dtype=torch.float32).pin_memory(), torch.zeros(1, dtype=torch.int64).pin_memory()) for _ in xs]
+    for p, o in zip(pins, outs):
+        pipe.submit(p, cfg.r, *o)
+    pipe.wait()
+    for x, (s, d, q, c) in zip(xs, outs):
+        exp = oracle.frnn(x, cfg.r, cfg.k_max)
+        e = int(c.item())
+        assert e == exp.count
+        assert_same(Got(s[:e].numpy(), d[:e].numpy(), q[:e].numpy()), exp, cfg.r, "host pipeline")
+    # capacity overflow is reported through the count word; pageable outputs are refused
+    small = F.HostPipeline(cfg.n, cfg.k_max, 1000, depth=1)
+    small.submit(pins[0], cfg.r, *outs[0])
+    small.wait()
+    assert int(outs[0][3].item()) == -oracle.frnn(xs[0], cfg.r, cfg.k_max).count - 1
+    with pytest.raises(F.FrnnError):
+        pipe.submit(pins[0], cfg.r, torch.empty(cap, dtype=torch.int32), outs[0][1], outs[0][2], outs[0][3])
+    small.close()
+    pipe.close()
