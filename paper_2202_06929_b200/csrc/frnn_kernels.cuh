@@ -377,6 +377,7 @@ constexpr int kSearchThreads = 128;
 #endif
 constexpr int kBatch = FRNN_KBATCH;    // candidates of a run tested per batch
 constexpr int kQueue = 32;             // survivor queue entries per thread (>= 2 * 3 * kBatch)
+constexpr int kLeft = 15;              // leftover-run entries per thread (the runs of 5 sub-batches)
 constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
 #ifndef FRNN_EMIT_THREADS
 #define FRNN_EMIT_THREADS 256
@@ -421,6 +422,21 @@ __device__ __forceinline__ void filter_push(uint32_t& qaddr, uint32_t key_a, uin
         : "memory");
 }
 
+// The part of a run beyond its first kBatch candidates, (first slot, length), goes on the thread's leftover
+// list if it is not empty: predicated 64-bit store and pointer bump, no branch.
+__device__ __forceinline__ void leftover_push(uint32_t& laddr, uint32_t j0, uint32_t len) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t.reg .u32 j, n;\n\t"
+        "setp.gt.u32 p, %2, %3;\n\t"
+        "add.u32 j, %1, %3;\n\t"
+        "sub.u32 n, %2, %3;\n\t"
+        "@p st.shared.v2.u32 [%0], {j, n};\n\t"
+        "@p add.u32 %0, %0, %4;\n\t}"
+        : "+r"(laddr)
+        : "r"(j0), "r"(len), "n"(kBatch), "n"(kSearchThreads * 8)
+        : "memory");
+}
+
 template <int G>
 __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search_kernel(SearchArgs a) {
     constexpr int NU = G >= 2 ? 3 : 1;                    // unrolled offsets of coordinate G-2
@@ -428,6 +444,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     constexpr int MID = (NB - 1) / 2;                     // the sub-batch with all-zero offsets
     constexpr int kWide = 4;                              // survivors evaluated together (rows in flight per thread)
     __shared__ uint32_t s_queue[kQueue][kSearchThreads];
+    __shared__ __align__(8) uint2 s_left[kLeft][kSearchThreads];      // leftover runs (first slot, length), one column per thread
     stamp_begin(a.stamps, 3);
     const int tid = threadIdx.x;
     const int64_t s64 = static_cast<int64_t>(blockIdx.x) * kSearchThreads + tid;
@@ -459,6 +476,9 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     const uint32_t q_base = static_cast<uint32_t>(__cvta_generic_to_shared(&s_queue[0][tid]));
     uint32_t qaddr = q_base;                              // shared-memory address of the next free queue entry
     constexpr uint32_t kQBytes = kSearchThreads * 4;      // one queue entry further down the thread's column
+    const uint32_t l_base = static_cast<uint32_t>(__cvta_generic_to_shared(&s_left[0][tid]));
+    uint32_t laddr = l_base;                              // shared-memory address of the next free leftover entry
+    constexpr uint32_t kLBytes = kSearchThreads * 8;
 
     // phase 2: evaluate the queued survivors (never the query itself), kWide at a time: kWide 256-bit row
     // loads in flight, then the R3 chains, then -- for the hits (i, j, d2) -- ONE returning atomic on cnt[i]
@@ -522,6 +542,32 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
             for (int v = 0; v < kBatch; ++v) filter_push(qaddr, key_a, kr[v], j0 + v);
         }
     };
+    // the merged loop over the listed leftovers: every iteration each lane with work left tests kBatch candidates
+    auto scan_leftovers = [&]() {
+        uint32_t la = l_base, cj0 = 0, cn = 0;
+        while (true) {
+            if (cn == 0u) {
+                if (la == laddr) break;
+                uint32_t x, y;
+                asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(x), "=r"(y) : "r"(la));
+                cj0 = x; cn = y;
+                la += kLBytes;
+            }
+            if (qaddr - q_base > (kQueue - kBatch) * kQBytes) drain();
+            const uint32_t* kp = a.skey + cj0;
+            uint32_t kr[kBatch];
+#pragma unroll
+            for (int v = 0; v < kBatch; ++v) {
+                kr[v] = key_fail;
+                if (static_cast<uint32_t>(v) < cn) kr[v] = kp[v];
+            }
+#pragma unroll
+            for (int v = 0; v < kBatch; ++v) filter_push(qaddr, key_a, kr[v], cj0 + v);
+            cj0 += kBatch;
+            cn = cn > kBatch ? cn - kBatch : 0u;
+        }
+        laddr = l_base;
+    };
     // general form: padded table index of cell 0 of the neighbour row with coordinates 0..G-3 offset by the
     // base-3 digits of b (coordinate 0 most significant) and coordinate G-2 by u - 1, all wrapped
     auto row_of = [&](int b, int u) -> uint32_t {
@@ -578,15 +624,13 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
         for (int u = 0; u < NU; ++u)
 #pragma unroll
             for (int v = 0; v < kBatch; ++v) filter_push(qaddr, key_a, kc[u][v], rs[u] + v);
-        // runs longer than kBatch: ONE copy of the loop (the run is picked with selects so rs/re stay in registers)
-        for (int t = 0; t < NU; ++t) {
-            uint32_t j0 = rs[0] + kBatch, j1 = re[0];
+        // what is left of runs longer than kBatch is listed now and filtered later, in ONE loop for all the rows
+        // (the lanes of a warp have their long runs in different rows: merged, they iterate together)
 #pragma unroll
-            for (int w = 1; w < NU; ++w)
-                if (t == w) { j0 = rs[w] + kBatch; j1 = re[w]; }
-            scan_run(j0, j1);
-        }
+        for (int u = 0; u < NU; ++u) leftover_push(laddr, rs[u], re[u] - rs[u]);
+        if (laddr - l_base > (kLeft - NU) * kLBytes) scan_leftovers();
     }
+    scan_leftovers();
     // Slots whose cell touches the seam of the torus in the last coordinate (only points beyond +-2^(bits-1)
     // cells from the origin) also visit the wrapped cell of every forward row: cold code.
     if (c_last == 0u || c_last == mask) {
