@@ -373,7 +373,7 @@ constexpr int kSearchThreads = 128;
 #define FRNN_SEARCH_MIN_BLOCKS 7       // 7 x 128 threads: 72 registers per thread; 7 x 148 blocks >= one 120k-point event
 #endif
 #ifndef FRNN_KBATCH
-#define FRNN_KBATCH 3
+#define FRNN_KBATCH 4
 #endif
 constexpr int kBatch = FRNN_KBATCH;    // candidates of a run tested per batch
 constexpr int kQueue = 32;             // survivor queue entries per thread (>= 2 * 3 * kBatch)
