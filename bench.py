@@ -184,6 +184,7 @@ def main() -> None:
     ap.add_argument("--e2e-steps", type=int, default=1000)
     ap.add_argument("--profile-steps", type=int, default=200)
     ap.add_argument("--timeline-steps", type=int, default=100)
+    ap.add_argument("--other-reps", type=int, default=50, help="repetitions for the other configs / N sweep (0: skip)")
     ap.add_argument("--next-steps", type=int, default=300, help="timed repetitions of the two edge-list consumers (0: skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -317,7 +318,7 @@ def main() -> None:
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                "kernel_us": dom_us, "note": "candidate rows are served by L2/L1, so this is an HBM-equivalent rate"}
+                "kernel_us": dom_us, "kernel_us_in_graph": (timeline_us or {}).get(dom, {}).get("dur"), "note": "candidate rows are served by L2/L1, so this is an HBM-equivalent rate"}
     path_bytes = cand * 32.0 + 12.0 * e_mean
     path_bytes_g3 = cand_g3 * 32.0 + 12.0 * e_mean
     t_event = ms_local / args.steps * 1e-3          # this rank's seconds per event
@@ -366,6 +367,58 @@ def main() -> None:
             "label_components": {"us_per_event": l_us, "nodes": n, "edges": e_mean, "threshold": 0.5,
                                  "components": int(ncomp.item()), "note": "3 kernels: init, hook (CAS union-find), flatten"},
         }
+
+    # the other BASELINE configs and the N sweep ("inference time depends almost linearly on the number
+    # of spacepoints"): same call, CUDA events around back-to-back replays of ONE input (so L2 is warm for the small ones)
+    other = None
+    if args.other_reps > 0:
+        import dataclasses
+
+        def time_single(x_np, cfg_r, cfg_k, reps):
+            p = torch.from_numpy(x_np).to(dev)
+            w = F.Workspace(len(x_np), 1, cfg_k, max(len(x_np) * EDGE_CAP_PER_ROW, 64), dev)
+            with torch.cuda.stream(stream):
+                for _ in range(5):
+                    F.frnn_build_ex(p, cfg_r, cfg_k, ws=w, stream=stream)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(reps):
+                    F.frnn_build_ex(p, cfg_r, cfg_k, ws=w, stream=stream)
+                b.record(stream)
+                stream.synchronize()
+            assert int(w.status.item()) == 0
+            return a.elapsed_time(b) / reps, int(w.count.item())
+
+        other = {}
+        for idx, reps in ((0, 20 * args.other_reps), (1, 20 * args.other_reps), (4, args.other_reps)):
+            c = events.CONFIGS[idx]
+            ms, e = time_single(events.make_event(c), c.r, c.k_max, reps)
+            other[c.name] = {"n": c.n, "ms_per_event": ms, "edges": e, "edges_per_s": e / (ms * 1e-3), "grid": F.frnn_get_grid(c.n, 1)}
+        c3 = events.CONFIGS[3]
+        xb, offs = events.make_batch(c3)
+        pb = torch.from_numpy(xb).to(dev)
+        wb = F.Workspace(len(xb), c3.n_events, c3.k_max, len(xb) * 4, dev)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                F.frnn_build_batched(pb, offs, c3.r, c3.k_max, ws=wb, stream=stream)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(args.other_reps):
+                F.frnn_build_batched(pb, offs, c3.r, c3.k_max, ws=wb, stream=stream)
+            b.record(stream)
+            stream.synchronize()
+        assert int(wb.status.item()) == 0
+        ms3 = a.elapsed_time(b) / args.other_reps
+        e3 = int(wb.count[-1].item())
+        other[c3.name] = {"n": len(xb), "events": c3.n_events, "ms_per_batch": ms3, "ms_per_event": ms3 / c3.n_events, "edges": e3,
+                          "edges_per_s": e3 / (ms3 * 1e-3), "grid": F.frnn_get_grid(len(xb), c3.n_events)}
+        del pb, wb
+        sweep = []
+        for nn in (15000, 30000, 60000, 120000):
+            c = dataclasses.replace(CFG, n=nn, n_tracks=CFG.n_tracks * nn // CFG.n)
+            ms, e = time_single(events.make_event(c, 77), c.r, c.k_max, 10 * args.other_reps)
+            sweep.append({"n": nn, "ms_per_event": ms, "edges": e, "us_per_1k_points": 1e3 * ms / (nn / 1000)})
+        other["n_sweep_config2_recipe"] = sweep
 
     # end to end through the host-buffer entry point: pinned host buffers, copies inside the timed region
     e2e = None
@@ -435,7 +488,7 @@ def main() -> None:
                              f"{len(seeds) * cap * 12 / 1e6:.0f} MB out > 126 MB L2); no explicit flush",
                        "grid": {"dims": dims, "bits": bits}, "edge_capacity": cap, "parallelism": f"events sharded over {rank.world_size} GPU(s), no collective"},
             "edges_per_event": e_mean, "roofline": roofline, "path_roofline": path_roofline, "phases_us": phases_us, "timeline_us": timeline_us,
-            "cpu_baseline": cpu_baseline, "e2e": e2e, "next_rows": next_rows, "gpu_launches": launches_per_step * args.steps,
+            "cpu_baseline": cpu_baseline, "e2e": e2e, "next_rows": next_rows, "other_configs": other, "gpu_launches": launches_per_step * args.steps,
             "gpu_launches_per_step": launches_per_step, "clocks": clocks,
             "host_wall_ms_per_step": 1e3 * (t1 - t0) / args.steps,
             "paper_context": "paper: 0.04 +- 0.01 s/event on V100 16 GB (PAPER.md:77 Table 1 'FRNN' column), TrackML events; other machine, other data",

@@ -18,6 +18,7 @@ using namespace frnn;
 
 constexpr float kCellSlack = 1.0078125f;   // 1 + 2^-7, see cell_coord()
 constexpr size_t kAlign = 256;
+constexpr int64_t kPrefixTilesMin = 1024;   // above this many emit tiles the tile offsets come from tile_prefix_kernel
 
 int g_force_dims = 0, g_force_bits = 0;
 int g_use_graph = 1;
@@ -63,7 +64,7 @@ struct Layout {
     int rows_per_block;
     int64_t scan_blocks;
     size_t off_cells, off_tiles, off_counters, zero_bytes;
-    size_t off_pcell, off_prank, off_spts, off_sidx, off_skey, off_cnt, off_evoff, off_hits;
+    size_t off_pcell, off_prank, off_spts, off_sidx, off_skey, off_cnt, off_evoff, off_hits, off_tprefix;
     size_t total;
 };
 
@@ -90,6 +91,7 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     L.off_sidx = o;   o = align_up(o + n * 4);
     L.off_skey = o;   o = align_up(o + n * 4);
     L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
+    L.off_tprefix = o; o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8);
     L.off_hits = o;   o = align_up(o + n * kSlot * sizeof(int2));
     L.total = o;
     return L;
@@ -206,10 +208,16 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
 
     EmitArgs ea;
     ea.pts = pts; ea.spts = spts; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
-    ea.tile_deg = tile_deg; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
+    ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
     ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps;
+    if (L.emit_tiles > kPrefixTilesMin) {                      // many tiles: their prefix in one small kernel (see tile_prefix_kernel)
+        unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
+        tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
+        ++t_launches; CK(cudaGetLastError());
+        ea.tile_prefix = tprefix;
+    }
     FRNN_DISPATCH_G(G, (emit_kernel<GG><<<static_cast<unsigned>(L.emit_tiles), kEmitThreads, 0, st>>>(ea)));
     ++t_launches; CK(cudaGetLastError());
     mark(5, st);

@@ -651,6 +651,51 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
 }
 
 // ------------------------------------------------------------------------------------------------
+// S9 for calls with many emit tiles (batches, million-point events): exclusive prefix of the per-tile totals in
+// ONE block, so that emit_kernel reads one value per block instead of summing all earlier tiles itself (which is
+// quadratic in the number of tiles).  Calls with few tiles skip this kernel: one dependent launch less.
+// ------------------------------------------------------------------------------------------------
+constexpr int kPrefixThreads = 1024;
+__global__ void __launch_bounds__(kPrefixThreads) tile_prefix_kernel(const unsigned long long* __restrict__ tile_deg, uint32_t n_tiles,
+                                                                     unsigned long long* __restrict__ tile_prefix) {
+    __shared__ unsigned long long s_w[kPrefixThreads / 32];
+    __shared__ unsigned long long s_carry;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    for (uint32_t c0 = 0; c0 < n_tiles; c0 += kPrefixThreads) {          // chunks of 1024 tiles, coalesced loads
+        const uint32_t t = c0 + threadIdx.x;
+        unsigned long long part[kDegSlices], mine = 0;
+#pragma unroll
+        for (int sl = 0; sl < kDegSlices; ++sl) part[sl] = t < n_tiles ? tile_deg[static_cast<size_t>(sl) * n_tiles + t] : 0ull;
+#pragma unroll
+        for (int sl = 0; sl < kDegSlices; ++sl) mine += part[sl];
+        unsigned long long incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long x = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += x;
+        }
+        if (lane == 31) s_w[warp] = incl;
+        __syncthreads();
+        unsigned long long wsum = lane < kPrefixThreads / 32 ? s_w[lane] : 0ull;   // scan of the 32 warp totals in every warp
+        unsigned long long wincl = wsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long x = __shfl_up_sync(kFull, wincl, o);
+            if (lane >= o) wincl += x;
+        }
+        const unsigned long long before_warp = __shfl_sync(kFull, wincl - wsum, warp);
+        const unsigned long long total = __shfl_sync(kFull, wincl, 31);
+        const unsigned long long carry = s_carry;
+        if (t < n_tiles) tile_prefix[t] = carry + before_warp + (incl - mine);
+        __syncthreads();
+        if (threadIdx.x == 0) s_carry = carry + total;
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // S8-S10: emit.  Thread per row in ORIGINAL order.  The search pass left sum(min(|S_i|, k_max)) per
 // 512-row tile in tile_deg, so a block gets its global edge offset by summing the totals of the
 // tiles before it (no inter-block wait), scans its own capped degrees -> CSR row_ptr, and every row
@@ -699,6 +744,7 @@ struct EmitArgs {
     const uint32_t* cnt;
     const int2* hits;
     const unsigned long long* tile_deg;
+    const unsigned long long* tile_prefix;   // exclusive prefix of the tile totals (tile_prefix_kernel), or NULL: sum in the block
     const int64_t* ev_off;        // device event offsets (n_events + 1) or NULL for one event
     int n_events;
     int64_t n_total;
@@ -798,8 +844,8 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     const uint32_t c = has ? a.cnt[i] : 0u;
     const uint32_t deg = c < a.k_max ? c : a.k_max;
     // ---- global offset of the tile = sum of the totals of the tiles before it
-    unsigned long long before = 0;
-    for (uint32_t t = threadIdx.x; t < tile; t += kEmitThreads) {
+    unsigned long long before = (a.tile_prefix && threadIdx.x == 0) ? a.tile_prefix[tile] : 0ull;
+    for (uint32_t t = threadIdx.x; t < (a.tile_prefix ? 0u : tile); t += kEmitThreads) {
         unsigned long long part[kDegSlices];
 #pragma unroll
         for (int sl = 0; sl < kDegSlices; ++sl) part[sl] = a.tile_deg[static_cast<size_t>(sl) * gridDim.x + t];      // all in flight
@@ -873,9 +919,11 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
         const uint32_t m = static_cast<uint32_t>(p - r0);
         const int64_t row = tile_row0 + r;
         const int2* h = a.hits + row * kSlot;
+        const int4 v0 = *reinterpret_cast<const int4*>(h);             // hits 0..3 and mine: three loads in flight (the
+        const int4 v1 = *reinterpret_cast<const int4*>(h + 2);         // slot buffer is padded, unused slots are masked)
         const int2 mine = h[m];
-        uint32_t rank = 0;
-        for (uint32_t u = 0; u < cr; u += 2) {                         // two hits per 16-byte load (slot buffers are padded)
+        uint32_t rank = (v0.x < mine.x) + (1u < cr && v0.z < mine.x) + (2u < cr && v1.x < mine.x) + (3u < cr && v1.z < mine.x);
+        for (uint32_t u = 4; u < cr; u += 2) {                         // two hits per 16-byte load
             const int4 v = *reinterpret_cast<const int4*>(h + u);
             rank += (v.x < mine.x) + (u + 1 < cr && v.z < mine.x);
         }
