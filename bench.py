@@ -358,7 +358,13 @@ def main() -> None:
             F.frnn_label_components(n, outs[k].src, outs[k].dst, score=scores, threshold=0.5, edge_count=outs[k].count,
                                     edge_max=e_cap, labels=labels, n_components=ncomp, stream=stream)
 
+        def dense(i):
+            k = i % len(outs)
+            F.frnn_build_dense_ex(pts[k], r, k_max, ws=outs[k], stream=stream)
+
         g_us, l_us = t_loop(gather, args.next_steps), t_loop(label, args.next_steps)
+        d_us = t_loop(dense, max(args.next_steps // 50, 3))
+        assert [int(w.count.item()) for w in outs[:3]] == edges_per_event[:3], "brute-force variant disagrees with the grid path"
         g_bytes = e_mean * (8 + 64 + 64)
         next_rows = {
             "gather_edge_rows": {"us_per_event": g_us, "edges": e_mean, "algorithmic_bytes": g_bytes,
@@ -366,6 +372,13 @@ def main() -> None:
                                  "note": "per edge: 8 B indices + 2 x 32 B rows read (L2) + 64 B written (streaming stores)"},
             "label_components": {"us_per_event": l_us, "nodes": n, "edges": e_mean, "threshold": 0.5,
                                  "components": int(ncomp.item()), "note": "3 kernels: init, hook (CAS union-find), flatten"},
+            "dense_bruteforce": {"ms_per_event": d_us * 1e-3, "pair_evaluations": n * (n - 1) / 2,
+                                 "pairs_per_s": n * (n - 1) / 2 / (d_us * 1e-6), "slower_than_grid_path": d_us * 1e-3 / ms_per_step,
+                                 "bound": "alu", "fp32_lane_instr_per_s": 16 * n * (n - 1) / 2 / (d_us * 1e-6),
+                                 "fp32_peak_lane_instr_per_s": 148 * 128 * 1.965e9,
+                                 "frac_of_fp32_issue_peak": 16 * n * (n - 1) / 2 / (d_us * 1e-6) / (148 * 128 * 1.965e9),
+                                 "note": "frnn_build_dense_ex: every unordered pair once, same R3 chain; the paper's own ratio "
+                                         "flat-index kNN + cut : grid FRNN is 0.54 s : 0.04 s (PAPER.md:77, V100)"},
         }
 
     # the other BASELINE configs and the N sweep ("inference time depends almost linearly on the number

@@ -113,6 +113,18 @@ int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * The brute-force variant.  PAPER.md:57 (section 3.1): the graph can be built by querying every
+ * point against a flat index (no grid) and cutting the neighbours at the radius; "brute force ...
+ * quadratic".  Same arguments, same result (bit for bit) and same error behaviour as frnn_build_ex: the K nearest
+ * within r of a flat search ARE the K-capped radius neighbourhood.  Cost O(n^2): every unordered pair is evaluated
+ * once; meant as the on-GPU second opinion and as the baseline the grid is measured against.  n <= 8,388,480.
+ */
+int frnn_build_dense_ex(const float* points, int64_t n, int dim, float r, int k_max,
+                        int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                        int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
  * Batched events (BASELINE.json config 3): n_events independent events concatenated in `points`;
  * event e owns rows [event_offsets[e], event_offsets[e+1]) (HOST int64[n_events+1], ascending,
  * event_offsets[0] == 0).  No cross-event edges.  src/dst are LOCAL to the event.  Edges of event

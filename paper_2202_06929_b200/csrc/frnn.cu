@@ -138,11 +138,12 @@ struct Call {                 // everything that determines the enqueued work (a
     int grid_dims, grid_bits;
     std::vector<int64_t> ev_off;
     bool timeline = false;
+    bool dense = false;           // frnn_build_dense_ex: brute force instead of the grid
     bool operator==(const Call& o) const {
         return points == o.points && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
                out_dst == o.out_dst && out_d2 == o.out_d2 && capacity == o.capacity && out_count == o.out_count &&
                out_edge_offsets == o.out_edge_offsets && out_status == o.out_status && out_row_ptr == o.out_row_ptr &&
-               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline;
+               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline && dense == o.dense;
     }
 };
 
@@ -170,6 +171,30 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     const float inv_cell = 1.0f / cell_side;
 
     mark(-1, st);
+    if (c.dense) {                                             // brute force: no table, no sort (single event)
+        CK(cudaMemsetAsync(ws + L.off_tiles, 0, L.zero_bytes - L.off_tiles, st)); ++t_launches;
+        DenseArgs da;
+        da.pts = pts; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = static_cast<uint32_t>(L.emit_tiles);
+        da.n = n_total; da.r2 = r2; da.k_max = static_cast<uint32_t>(c.k_max);
+        const unsigned T = static_cast<unsigned>((n_total + kDenseTile - 1) / kDenseTile);
+        dense_search_kernel<<<dim3(T, T), kDenseTile, 0, st>>>(da);
+        ++t_launches; CK(cudaGetLastError());
+        EmitArgs ea;
+        ea.pts = pts; ea.spts = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.cnt = cnt; ea.hits = hits; ea.ev_off = nullptr;
+        ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = 1; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
+        ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
+        ea.out_edge_offsets = nullptr; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
+        ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = nullptr; ea.dense = 1;
+        if (L.emit_tiles > kPrefixTilesMin) {
+            unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
+            tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
+            ++t_launches; CK(cudaGetLastError());
+            ea.tile_prefix = tprefix;
+        }
+        emit_kernel<1><<<static_cast<unsigned>(L.emit_tiles), kEmitThreads, 0, st>>>(ea);
+        ++t_launches; CK(cudaGetLastError());
+        return FRNN_OK;
+    }
     CK(cudaMemsetAsync(ws, 0, L.zero_bytes, st)); ++t_launches;
     // Event offsets reach the device as kernel arguments (no pageable-memory copy, which would
     // synchronise the host with the stream); a single event needs none (base 0).
@@ -211,7 +236,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
-    ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps;
+    ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps; ea.dense = 0;
     if (L.emit_tiles > kPrefixTilesMin) {                      // many tiles: their prefix in one small kernel (see tile_prefix_kernel)
         unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
         tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
@@ -369,6 +394,20 @@ int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
     if (rc != FRNN_OK) return rc;
     if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
     Call c{points, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
+    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
+    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int frnn_build_dense_ex(const float* points, int64_t n, int dim, float r, int k_max,
+                        int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                        int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    if (rc != FRNN_OK) return rc;
+    if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
+    if (n > 65535ll * kDenseTile) return FRNN_ERR_UNSUPPORTED;                 // grid.y limit (8.3 M rows)
+    Call c{points, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
+    c.dense = true;
     if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
     return run_call(c, static_cast<cudaStream_t>(cuda_stream));
 }

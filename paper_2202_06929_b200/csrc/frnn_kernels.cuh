@@ -651,6 +651,58 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
 }
 
 // ------------------------------------------------------------------------------------------------
+// the brute-force variant (section 3.1: flat-index nearest neighbours followed by
+// the radius cut; "brute force ... quadratic").  Every unordered pair of the event is evaluated once
+// with the same R3 chain; block (I, J), J >= I, holds 128 queries in registers and 128 candidate rows in shared
+// memory (read back as broadcasts).  Hits go through the same slot buffers, counters and per-tile totals as the
+// grid path, so emit_kernel (K cap, ordering, compaction) is shared.
+// ------------------------------------------------------------------------------------------------
+constexpr int kDenseTile = 128;
+struct DenseArgs {
+    const float4* pts;
+    uint32_t* cnt;
+    int2* hits;
+    unsigned long long* tile_deg;
+    uint32_t n_tiles;
+    int64_t n;
+    float r2;
+    uint32_t k_max;
+};
+
+__global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
+    const uint32_t I = blockIdx.y, J = blockIdx.x;
+    if (J < I) return;
+    __shared__ float4 s_c[kDenseTile][2];
+    const int tid = threadIdx.x;
+    const int64_t i = static_cast<int64_t>(I) * kDenseTile + tid;
+    const int64_t jr = static_cast<int64_t>(J) * kDenseTile + tid;
+    float4 qa = make_float4(0.f, 0.f, 0.f, 0.f), qb = qa;
+    if (i < a.n) load_row_nc(a.pts + 2 * i, qa, qb);
+    float4 ca = make_float4(__int_as_float(0x7f800000), 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (jr < a.n) load_row_nc(a.pts + 2 * jr, ca, cb);                 // rows beyond the event: +inf, never within r
+    s_c[tid][0] = ca; s_c[tid][1] = cb;
+    __syncthreads();
+    if (i >= a.n) return;
+    unsigned long long* const my_tile_deg = a.tile_deg + static_cast<size_t>(J & (kDegSlices - 1)) * a.n_tiles;
+    const int k0 = I == J ? tid + 1 : 0;                               // own tile: only the rows after mine
+    const int32_t row = static_cast<int32_t>(i);
+#pragma unroll 4
+    for (int k = k0; k < kDenseTile; ++k) {
+        const float d2 = d2_pinned(qa, qb, s_c[k][0], s_c[k][1]);
+        if (d2 <= a.r2) {
+            const int32_t cj = static_cast<int32_t>(J * kDenseTile + k);
+            const int d2b = __float_as_int(d2);
+            const uint32_t p0 = atomicAdd(&a.cnt[row], 1u);
+            const uint32_t p1 = atomicAdd(&a.cnt[cj], 1u);
+            if (p0 < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + p0] = make_int2(cj, d2b);
+            if (p1 < kSlot) a.hits[static_cast<int64_t>(cj) * kSlot + p1] = make_int2(row, d2b);
+            if (p0 < a.k_max) atomicAdd(&my_tile_deg[row / kEmitThreads], 1ull);
+            if (p1 < a.k_max) atomicAdd(&my_tile_deg[cj / kEmitThreads], 1ull);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // S9 for calls with many emit tiles (batches, million-point events): exclusive prefix of the per-tile totals in
 // ONE block, so that emit_kernel reads one value per block instead of summing all earlier tiles itself (which is
 // quadratic in the number of tiles).  Calls with few tiles skip this kernel: one dependent launch less.
@@ -760,6 +812,7 @@ struct EmitArgs {
     float r2, inv_cell;
     int bits;
     uint32_t k_max;
+    int dense;                    // 1: no grid exists (frnn_build_dense_ex): recomputed rows scan their whole event
 };
 
 template <int G, bool INTERIOR>
@@ -769,6 +822,17 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
     const float inf = __int_as_float(0x7f800000);
     // visit(g): g(in_radius, j, d2) once per chunk, one candidate per lane
     auto visit = [&](auto&& g) {
+        if (a.dense) {                                    // every row of the event, 32 at a time, in original order
+            const int64_t ev_end = a.ev_off ? a.ev_off[event_of_row(a.ev_off, a.n_events, row) + 1] : a.n_total;
+            for (int64_t j0 = row_ev; j0 < ev_end; j0 += 32) {
+                const int64_t j = j0 + lane;
+                float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (j < ev_end) { ca = a.pts[2 * j]; cb = a.pts[2 * j + 1]; }
+                const float d2 = d2_pinned(qa, qb, ca, cb);
+                g(j < ev_end && d2 <= a.r2 && j != row, static_cast<int32_t>(j), d2);
+            }
+            return;
+        }
         for_each_candidate_chunk<G, INTERIOR>(cell, a.bits, lane_delta, a.cell_start, s_delta, lane, [&](int cslot) {
             float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
             int32_t cj = -1;

@@ -34,6 +34,10 @@ _SIGNATURES = {
                                  _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
                                  _c.c_void_p, _c.c_void_p, _c.c_void_p,
                                  _c.c_void_p, _c.c_size_t, _c.c_void_p]),
+    "frnn_build_dense_ex": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
+                                       _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
+                                       _c.c_void_p, _c.c_void_p, _c.c_void_p,
+                                       _c.c_void_p, _c.c_size_t, _c.c_void_p]),
     "frnn_build_batched": (_c.c_int, [_c.c_void_p, _c.POINTER(_c.c_int64), _c.c_int, _c.c_int, _c.c_float, _c.c_int,
                                       _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
                                       _c.c_void_p, _c.c_void_p, _c.c_void_p,
@@ -204,9 +208,16 @@ class Workspace:
         self.row_ptr = torch.empty(n_total + 1, dtype=torch.int64, device=device) if want_row_ptr else None
 
 
+def frnn_build_dense_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int | None = None,
+                        ws: Workspace | None = None, stream: torch.cuda.Stream | None = None,
+                        want_row_ptr: bool = False) -> EdgeList:
+    """The brute-force variant of ``frnn_build_ex``: same result, O(n^2)."""
+    return frnn_build_ex(points, r, k_max, edge_capacity, ws, stream, want_row_ptr, _entry="frnn_build_dense_ex")
+
+
 def frnn_build_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int | None = None,
                   ws: Workspace | None = None, stream: torch.cuda.Stream | None = None,
-                  want_row_ptr: bool = False) -> EdgeList:
+                  want_row_ptr: bool = False, _entry: str = "frnn_build_ex") -> EdgeList:
     """Asynchronous single-event build on ``stream`` (default: torch's current stream)."""
     _require_cuda(points)
     n, dim = points.shape
@@ -215,10 +226,10 @@ def frnn_build_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int
     if ws is None:
         ws = Workspace(n, 1, k_max, edge_capacity, points.device, want_row_ptr)
     stream = stream or torch.cuda.current_stream(points.device)
-    st = lib().frnn_build_ex(_ptr(points), n, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst), _ptr(ws.d2),
-                             int(edge_capacity), _ptr(ws.count), _ptr(ws.status), _ptr(ws.row_ptr),
-                             _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
-    _check(st, "frnn_build_ex")
+    st = getattr(lib(), _entry)(_ptr(points), n, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst), _ptr(ws.d2),
+                                int(edge_capacity), _ptr(ws.count), _ptr(ws.status), _ptr(ws.row_ptr),
+                                _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    _check(st, _entry)
     return EdgeList(ws.src, ws.dst, ws.d2, ws.count, ws.status, ws.row_ptr)
 
 

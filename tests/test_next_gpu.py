@@ -155,3 +155,69 @@ def test_chain_build_gather_label_without_host_sync(F):
     assert np.array_equal(rows[:g.count].cpu().numpy(), NO.gather_edge_rows(x, g.src, g.dst))
     exp, nc_exp = NO.label_components(cfg.n, g.src, g.dst)
     assert np.array_equal(lab.cpu().numpy(), exp) and int(nc.item()) == nc_exp
+
+
+# ---------------------------------------------------------------- f1: the brute-force variant
+def run_dense(F, x, r, k, capacity=None, want_row_ptr=False):
+    pts = dev(x)
+    res = F.frnn_build_dense_ex(pts, r, k, edge_capacity=capacity, want_row_ptr=want_row_ptr)
+    torch.cuda.synchronize()
+    return res
+
+
+def same_as_oracle(res, exp):
+    res.check()
+    s, d, q = (t.cpu().numpy() for t in res.trimmed())
+    assert np.array_equal(s, exp.src) and np.array_equal(d, exp.dst)
+    assert np.array_equal(q.view(np.uint32), exp.d2.view(np.uint32))
+
+
+@pytest.mark.parametrize("cfg_idx", [0, 1, 2])
+def test_dense_configs(F, cfg_idx):
+    """Config 2 at full size: 7.2e9 pair evaluations on the GPU against the cell-list oracle."""
+    cfg = events.CONFIGS[cfg_idx]
+    x = events.make_event(cfg)
+    exp = oracle.frnn(x, cfg.r, cfg.k_max, oracle.CELLS)
+    res = run_dense(F, x, cfg.r, cfg.k_max, capacity=cfg.n * 8, want_row_ptr=True)
+    same_as_oracle(res, exp)
+    rp = res.row_ptr.cpu().numpy()
+    assert np.array_equal(np.diff(rp), np.minimum(exp.uncapped, cfg.k_max)) and rp[0] == 0
+
+
+@pytest.mark.parametrize("k", [1, 7, 64, 4096])
+def test_dense_one_cluster_k_cap(F, k):
+    x = events.one_cluster(2000, 0.01, 3)
+    same_as_oracle(run_dense(F, x, 0.1, k), oracle.frnn(x, 0.1, k, oracle.BRUTE))
+
+
+@pytest.mark.parametrize("fac,k", [(1.0, 1024), (1.8, 1024), (1.8, 100), (1.8, 1)])
+def test_dense_lattice_ties(F, fac, k):
+    x = events.lattice(3, 8, 0.125)
+    r = float(np.float32(fac * 0.125))
+    same_as_oracle(run_dense(F, x, r, k), oracle.frnn(x, r, k, oracle.BRUTE))
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 127, 128, 129, 300])
+def test_dense_ragged_sizes_and_duplicates(F, n):
+    x = events.uniform_points(max(n, 1), 8, -0.2, 0.2, n)[:n].copy()
+    if n > 5:
+        x[3] = x[0]; x[n - 1] = x[0]
+    exp = oracle.frnn(x, 0.15, 5, oracle.BRUTE)
+    res = run_dense(F, x, 0.15, 5, capacity=max(n * 5, 1))
+    same_as_oracle(res, exp)
+    same_as_oracle(run_dense(F, x, 0.0, 5, capacity=max(n * 5, 1)), oracle.frnn(x, 0.0, 5, oracle.BRUTE))
+
+
+def test_dense_equals_grid_and_reports_capacity(F):
+    cfg = events.CONFIGS[1]
+    x = events.make_event(cfg, 9)
+    pts = dev(x)
+    a = F.frnn_build_ex(pts, cfg.r, 3)
+    b = F.frnn_build_dense_ex(pts, cfg.r, 3)
+    torch.cuda.synchronize()
+    for u, v in zip(a.trimmed(), b.trimmed()):
+        assert torch.equal(u, v)
+    ws = F.Workspace(cfg.n, 1, cfg.k_max, 1000)
+    res = F.frnn_build_dense_ex(pts, cfg.r, cfg.k_max, edge_capacity=1000, ws=ws)
+    torch.cuda.synchronize()
+    assert int(res.status.item()) == F.FRNN_ERR_CAPACITY and res.n_edges() == oracle.frnn(x, cfg.r, cfg.k_max).count
