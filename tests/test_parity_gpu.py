@@ -319,3 +319,32 @@ def test_host_pipeline_overlapped_events(F):
         pipe.submit(pins[0], cfg.r, torch.empty(cap, dtype=torch.int32), outs[0][1], outs[0][2], outs[0][3])
     small.close()
     pipe.close()
+
+
+def test_canaries_around_workspace_and_outputs(F):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds WRITES are hunted with canaries: the workspace
+    and the three output arrays sit inside larger buffers filled with a pattern that must survive every call."""
+    L = F.lib()
+    cases = [(events.make_event(events.CONFIGS[0]), 0.1, 64), (events.make_event(events.CONFIGS[1]), 0.1, 3),
+             (events.one_cluster(2000, 0.01, 3), 0.1, 7), (events.lattice(3, 8, 0.125), float(np.float32(1.8 * 0.125)), 100)]
+    pad = 4096
+    for x, r, k in cases:
+        n = len(x)
+        exp = oracle.frnn(x, r, k, oracle.BRUTE if n <= 7000 else oracle.CELLS)
+        cap = exp.count                                                   # exactly enough room
+        wsb = F.frnn_workspace_bytes(n, 1, 8, k)
+        big_ws = torch.full((wsb + 2 * pad,), 0xA5, dtype=torch.uint8, device="cuda")
+        outs = [torch.full((cap + 2 * 1024,), -7, dtype=torch.int32, device="cuda") for _ in range(3)]
+        pts = torch.from_numpy(x).cuda()
+        cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+        stat = torch.zeros(1, dtype=torch.int32, device="cuda")
+        for entry in (L.frnn_build_ex, L.frnn_build_dense_ex):
+            rc = entry(pts.data_ptr(), n, 8, r, k, outs[0][1024:].data_ptr(), outs[1][1024:].data_ptr(), outs[2][1024:].data_ptr(), cap,
+                       cnt.data_ptr(), stat.data_ptr(), None, big_ws[pad:].data_ptr(), wsb, None)
+            torch.cuda.synchronize()
+            assert rc == 0 and int(stat.item()) == 0 and int(cnt.item()) == cap
+            assert bool((big_ws[:pad] == 0xA5).all()) and bool((big_ws[pad + wsb:] == 0xA5).all()), "write outside the workspace"
+            for o in outs:
+                assert bool((o[:1024] == -7).all()) and bool((o[1024 + cap:] == -7).all()), "write outside an output array"
+            assert np.array_equal(outs[0][1024:1024 + cap].cpu().numpy(), exp.src)
+            assert np.array_equal(outs[1][1024:1024 + cap].cpu().numpy(), exp.dst)
