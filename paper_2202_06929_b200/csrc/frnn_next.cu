@@ -26,8 +26,8 @@ __device__ __forceinline__ void store_row_cs(float4* p, const float4& a, const f
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// f4: one thread per (edge, end point): consecutive threads write consecutive 32-byte rows of `out` (fully
-// coalesced 256-bit stores); the point rows are random 32-byte sectors served by L2 (one event = 3.84 MB).
+// f4: one thread per edge: both indices, then both 256-bit row loads in flight (random 32-byte sectors served by L2:
+// one event = 3.84 MB), then 64 contiguous bytes stored; a warp writes 2 KB contiguous (streaming stores).
 // ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) gather_edge_rows_kernel(const float4* __restrict__ pts, int64_t n,
                                                                const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
@@ -35,16 +35,17 @@ __global__ void __launch_bounds__(256) gather_edge_rows_kernel(const float4* __r
                                                                int64_t row_base, float4* __restrict__ out) {
     int64_t e_end = e_begin + e_max;
     if (edge_count) { const int64_t c = *edge_count; e_end = c < e_end ? c : e_end; }
-    const int64_t n_items = e_end > e_begin ? 2 * (e_end - e_begin) : 0;
-    for (int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; t < n_items;
-         t += static_cast<int64_t>(gridDim.x) * blockDim.x) {
-        const int64_t e = e_begin + (t >> 1);
-        int64_t row = static_cast<int64_t>((t & 1) ? dst[e] : src[e]) + row_base;
-        row = row < 0 ? 0 : (row >= n ? n - 1 : row);             // indices are a precondition; never read out of bounds
-        float4 a, b;
-        load_row_nc(pts + 2 * row, a, b);
-        store_row_cs(out + 2 * t, a, b);
-    }
+    const int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const int64_t e = e_begin + t;
+    if (e >= e_end) return;
+    int64_t ra = static_cast<int64_t>(src[e]) + row_base, rb = static_cast<int64_t>(dst[e]) + row_base;
+    ra = ra < 0 ? 0 : (ra >= n ? n - 1 : ra);                     // indices are a precondition; never read out of bounds
+    rb = rb < 0 ? 0 : (rb >= n ? n - 1 : rb);
+    float4 a0, a1, b0, b1;
+    load_row_nc(pts + 2 * ra, a0, a1);
+    load_row_nc(pts + 2 * rb, b0, b1);
+    store_row_cs(out + 4 * t, a0, a1);
+    store_row_cs(out + 4 * t + 2, b0, b1);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -130,7 +131,7 @@ int frnn_gather_edge_rows(const float* points, int64_t n, int dim, const int32_t
     if (n == 0 || !points || !src || !dst || !out) return FRNN_ERR_INVALID_ARG;
     if (reinterpret_cast<uintptr_t>(points) % 32 || reinterpret_cast<uintptr_t>(out) % 32) return FRNN_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    gather_edge_rows_kernel<<<blocks_for(2 * e_max, 256, 148 * 64), 256, 0, st>>>(
+    gather_edge_rows_kernel<<<blocks_for(e_max, 256, 0x7fffffff), 256, 0, st>>>(
         reinterpret_cast<const float4*>(points), n, src, dst, edge_count, e_begin, e_max, row_base, reinterpret_cast<float4*>(out));
     return cudaGetLastError() == cudaSuccess ? FRNN_OK : FRNN_ERR_CUDA;
 }
