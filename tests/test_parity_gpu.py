@@ -348,3 +348,27 @@ def test_canaries_around_workspace_and_outputs(F):
                 assert bool((o[:1024] == -7).all()) and bool((o[1024 + cap:] == -7).all()), "write outside an output array"
             assert np.array_equal(outs[0][1024:1024 + cap].cpu().numpy(), exp.src)
             assert np.array_equal(outs[1][1024:1024 + cap].cpu().numpy(), exp.dst)
+
+
+def test_non_finite_coordinates_cannot_fault(F):
+    """include/frnn.h: non-finite coordinates are a precondition violation but can never cause an out-of-bounds
+    access.  The result is unspecified for the affected rows; the call must complete, report a consistent count and
+    leave the rows that are far from every poisoned point exactly right."""
+    cfg = events.CONFIGS[0]
+    x = events.make_event(cfg).copy()
+    x[5, 0] = np.nan; x[77, 3] = np.inf; x[300, 7] = -np.inf; x[1000] = np.nan; x[2000, :4] = 3e38
+    for entry in (F.frnn_build_ex, F.frnn_build_dense_ex):
+        res = entry(torch.from_numpy(x).cuda(), cfg.r, cfg.k_max, edge_capacity=cfg.n * 8, want_row_ptr=True)
+        torch.cuda.synchronize()
+        res.check()
+        e = res.n_edges()
+        rp = res.row_ptr.cpu().numpy()
+        assert rp[0] == 0 and rp[-1] == e and np.all(np.diff(rp) >= 0)
+        s, d, _ = (t.cpu().numpy() for t in res.trimmed())
+        assert s.min() >= 0 and s.max() < cfg.n and d.min() >= 0 and d.max() < cfg.n
+        bad = np.zeros(cfg.n, bool); bad[[5, 77, 300, 1000, 2000]] = True
+        clean = events.make_event(cfg)
+        exp = oracle.frnn(clean, cfg.r, cfg.k_max)
+        keep_e = ~(bad[exp.src] | bad[exp.dst])
+        keep_g = ~(bad[s] | bad[d])
+        assert np.array_equal(s[keep_g], exp.src[keep_e]) and np.array_equal(d[keep_g], exp.dst[keep_e])
