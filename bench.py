@@ -184,6 +184,7 @@ def main() -> None:
     ap.add_argument("--e2e-steps", type=int, default=1000)
     ap.add_argument("--profile-steps", type=int, default=200)
     ap.add_argument("--timeline-steps", type=int, default=100)
+    ap.add_argument("--two-stream-steps", type=int, default=4000, help="steps of the two-events-in-flight throughput figure (0: skip)")
     ap.add_argument("--other-reps", type=int, default=50, help="repetitions for the other configs / N sweep (0: skip)")
     ap.add_argument("--next-steps", type=int, default=300, help="timed repetitions of the two edge-list consumers (0: skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -265,6 +266,33 @@ def main() -> None:
     value = total_edges / (ms * 1e-3)
     ms_per_step = ms / args.steps
     clocks = sampler.summary(t0, t1)
+    e_mean_all = float(np.mean(edges_per_event))
+
+    # throughput with two events in flight (two streams, two scratch workspaces): the fixed latency of one event's six
+    # dependent graph nodes overlaps the other event's work.  Reported beside the headline, which stays one stream.
+    two_streams = None
+    if args.two_stream_steps > 0:
+        stream_b = torch.cuda.Stream(dev)
+        scratch_b = torch.empty_like(shared)
+        args_b = [a[:12] + (C.c_void_p(scratch_b.data_ptr()), scratch_b.numel(), C.c_void_p(stream_b.cuda_stream)) for a in call_args]
+        for i in range(len(call_args)):                       # build the graphs of the second stream
+            assert build_ex(*args_b[i]) == 0
+        torch.cuda.synchronize()
+        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ea.record(stream)
+        stream_b.wait_event(ea)
+        for i in range(args.two_stream_steps):
+            k = i % len(call_args)
+            st = build_ex(*(call_args[k] if i % 2 == 0 else args_b[k]))     # outputs k are only touched by step i
+            assert st == 0
+        done_b = torch.cuda.Event()
+        done_b.record(stream_b)
+        stream.wait_event(done_b)
+        eb.record(stream)
+        torch.cuda.synchronize()
+        ms2 = ea.elapsed_time(eb) / args.two_stream_steps
+        two_streams = {"ms_per_event": ms2, "edges_per_s": e_mean_all / (ms2 * 1e-3), "steps": args.two_stream_steps,
+                       "note": "same call, events alternate between two streams with their own scratch workspace"}
 
     # per-phase device times (separate loop: event records between kernels perturb the main timing)
     phases = {}
@@ -501,7 +529,7 @@ def main() -> None:
                              f"{len(seeds) * cap * 12 / 1e6:.0f} MB out > 126 MB L2); no explicit flush",
                        "grid": {"dims": dims, "bits": bits}, "edge_capacity": cap, "parallelism": f"events sharded over {rank.world_size} GPU(s), no collective"},
             "edges_per_event": e_mean, "roofline": roofline, "path_roofline": path_roofline, "phases_us": phases_us, "timeline_us": timeline_us,
-            "cpu_baseline": cpu_baseline, "e2e": e2e, "next_rows": next_rows, "other_configs": other, "gpu_launches": launches_per_step * args.steps,
+            "cpu_baseline": cpu_baseline, "e2e": e2e, "next_rows": next_rows, "other_configs": other, "two_streams": two_streams, "gpu_launches": launches_per_step * args.steps,
             "gpu_launches_per_step": launches_per_step, "clocks": clocks,
             "host_wall_ms_per_step": 1e3 * (t1 - t0) / args.steps,
             "paper_context": "paper: 0.04 +- 0.01 s/event on V100 16 GB (PAPER.md:77 Table 1 'FRNN' column), TrackML events; other machine, other data",

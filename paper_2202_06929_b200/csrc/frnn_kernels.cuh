@@ -1,15 +1,17 @@
 // frnn_kernels.cuh -- device code of the B200 FRNN path (sm_100a).  Product code: shares nothing
 // with oracle/.  Steps S2..S10 of SURVEY.md section 8(a); design notes in DESIGN.md section 6.
 //
-//   bin_kernel      S2     cell index on a toroidal grid over the first G coordinates + histogram
-//   cell_scan_kernel S3    cell starts + list of occupied cells ("segments"); blocks take their base
-//                          from one atomic (no inter-block wait), rows of the table are padded so a
-//                          run never needs the next block's start
-//   scatter_kernel  S4     counting-sort scatter into the cell-ordered copy
-//   search_kernel   S5-S7  ONE pass: a warp per occupied cell, neighbour runs flattened across
-//                          lanes, whole 8-term FMA chains per lane; hits go to a per-row slot buffer
-//   emit_kernel     S8-S10 degree scan (decoupled look-back) fused with the per-row ordering by dst
-//                          and the compaction into the (src,dst)-sorted COO; exact K-cap selection
+//   bin_kernel       S2     cell index on a toroidal grid over the first G coordinates + histogram
+//   cell_scan_kernel S3     cell starts; blocks take their base from one atomic (no inter-block wait), rows of the
+//                           table are padded so a run never needs the next block's start
+//   scatter_kernel   S4     counting-sort scatter into the cell-ordered copy (256-bit row moves) + filter keys
+//   search_kernel    S5-S7  ONE pass, thread per query in cell order: 4-byte key filter on the unbinned coordinates,
+//                           every unordered pair evaluated once with whole 8-term FMA chains, hits appended to
+//                           per-row slot buffers of both end points
+//   tile_prefix_kernel S9   (only for calls with many emit tiles) exclusive prefix of the per-tile degree totals
+//   emit_kernel      S8-S10 block scan of the capped degrees, one thread per output edge (rank by dst): the
+//                           (src,dst)-sorted COO without a sort; exact K-cap selection for the rare big rows
+//   dense_search_kernel     SURVEY 8(f) f1: the brute-force variant, shares emit_kernel
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
