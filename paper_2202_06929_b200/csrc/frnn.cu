@@ -42,7 +42,7 @@ struct GridChoice { int dims, bits; };
 // Grid heuristic: cells per event = 2^(dims*bits).  Finer grids cut candidate rows per query
 // (3^dims cells of side ~r are visited) but cost table size and run bookkeeping; the switch points
 // come from the sweep recorded in DESIGN.md section 7.
-GridChoice choose_grid(int64_t n_total, int n_events) {
+GridChoice choose_grid(int64_t n_total, int n_events, int dim = kDim) {
     const int64_t per_event = n_events > 0 ? (n_total + n_events - 1) / n_events : n_total;
     GridChoice g;
     g.bits = g_force_bits ? g_force_bits : 5;
@@ -50,6 +50,7 @@ GridChoice choose_grid(int64_t n_total, int n_events) {
     else if (per_event < 16384) g.dims = 3;
     else if (per_event < 400000) g.dims = 4;
     else g.dims = 5;
+    if (!g_force_dims && g.dims > dim) g.dims = dim;          // binning a padded (all-zero) coordinate prunes nothing
     int ev_bits = 0;
     while ((1ll << ev_bits) < n_events) ++ev_bits;
     while (g.dims * g.bits + ev_bits > 30 && g.dims > 1) --g.dims;     // padded table index stays below 2^31
@@ -114,15 +115,16 @@ int check_common(const float* points, int64_t n, int dim, float r, int k_max, co
     if (n < 0 || k_max < 1 || capacity < 0) return FRNN_ERR_INVALID_ARG;
     if (!(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
     if (n > 0 && !points) return FRNN_ERR_INVALID_ARG;
-    if (reinterpret_cast<uintptr_t>(points) % 32) return FRNN_ERR_INVALID_ARG;      // rows move as 256-bit transactions
+    if (dim < 1 || dim > kDim) return FRNN_ERR_UNSUPPORTED;
+    if (reinterpret_cast<uintptr_t>(points) % (dim == kDim ? 32 : 4)) return FRNN_ERR_INVALID_ARG;   // 8-float rows move as 256-bit transactions
     if (capacity > 0 && (!out_src || !out_dst || !out_d2)) return FRNN_ERR_INVALID_ARG;
-    if (dim != kDim) return FRNN_ERR_UNSUPPORTED;
     if (n > 0x7fffffffll) return FRNN_ERR_UNSUPPORTED;
     return FRNN_OK;
 }
 
 struct Call {                 // everything that determines the enqueued work (also the graph-cache key)
     const float* points;
+    int dim = kDim;
     int n_events;
     float r;
     int k_max;
@@ -140,7 +142,7 @@ struct Call {                 // everything that determines the enqueued work (a
     bool timeline = false;
     bool dense = false;           // frnn_build_dense_ex: brute force instead of the grid
     bool operator==(const Call& o) const {
-        return points == o.points && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
+        return points == o.points && dim == o.dim && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
                out_dst == o.out_dst && out_d2 == o.out_d2 && capacity == o.capacity && out_count == o.out_count &&
                out_edge_offsets == o.out_edge_offsets && out_status == o.out_status && out_row_ptr == o.out_row_ptr &&
                workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline && dense == o.dense;
@@ -163,7 +165,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
     int64_t* ev_off = reinterpret_cast<int64_t*>(ws + L.off_evoff);
     int2* hits = reinterpret_cast<int2*>(ws + L.off_hits);
-    const float4* pts = reinterpret_cast<const float4*>(c.points);
+    const float* pts = c.points;
     const int G = c.grid_dims, bits = c.grid_bits;
 
     const float r2 = c.r * c.r;                               // R2: fl32(r*r), once, on the host
@@ -174,13 +176,13 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     if (c.dense) {                                             // brute force: no table, no sort (single event)
         CK(cudaMemsetAsync(ws + L.off_tiles, 0, L.zero_bytes - L.off_tiles, st)); ++t_launches;
         DenseArgs da;
-        da.pts = pts; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = static_cast<uint32_t>(L.emit_tiles);
+        da.pts = pts; da.dim = c.dim; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = static_cast<uint32_t>(L.emit_tiles);
         da.n = n_total; da.r2 = r2; da.k_max = static_cast<uint32_t>(c.k_max);
         const unsigned T = static_cast<unsigned>((n_total + kDenseTile - 1) / kDenseTile);
         dense_search_kernel<<<dim3(T, T), kDenseTile, 0, st>>>(da);
         ++t_launches; CK(cudaGetLastError());
         EmitArgs ea;
-        ea.pts = pts; ea.spts = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.cnt = cnt; ea.hits = hits; ea.ev_off = nullptr;
+        ea.pts = pts; ea.dim = c.dim; ea.spts = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.cnt = cnt; ea.hits = hits; ea.ev_off = nullptr;
         ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = 1; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
         ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
         ea.out_edge_offsets = nullptr; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
@@ -212,13 +214,13 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     }
     mark(0, st);
     const unsigned row_blocks = static_cast<unsigned>((n_total + 255) / 256);
-    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, stamps)));
+    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(1, st);
     cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor, stamps);
     ++t_launches; CK(cudaGetLastError());
     mark(2, st);
-    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, stamps)));
+    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(3, st);
 
@@ -232,7 +234,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     mark(4, st);
 
     EmitArgs ea;
-    ea.pts = pts; ea.spts = spts; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
+    ea.pts = pts; ea.dim = c.dim; ea.spts = spts; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
     ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
@@ -311,7 +313,7 @@ int run_call(const Call& c, cudaStream_t st) {
 
 int prepare(Call& c, size_t workspace_bytes) {
     const int64_t n_total = c.ev_off[c.n_events];
-    const GridChoice g = choose_grid(n_total, c.n_events);
+    const GridChoice g = choose_grid(n_total, c.n_events, c.dim);
     c.grid_dims = g.dims;
     c.grid_bits = g.bits;
     c.timeline = g_timeline;
@@ -355,7 +357,7 @@ const char* frnn_status_string(int status) {
     switch (status) {
         case FRNN_OK: return "ok";
         case FRNN_ERR_INVALID_ARG: return "invalid argument";
-        case FRNN_ERR_UNSUPPORTED: return "unsupported (dim != 8 or too many rows)";
+        case FRNN_ERR_UNSUPPORTED: return "unsupported (dim outside 1..8 or too many rows)";
         case FRNN_ERR_CAPACITY: return "edge capacity exceeded";
         case FRNN_ERR_WORKSPACE: return "workspace too small";
         case FRNN_ERR_CUDA: return "CUDA error";
@@ -364,8 +366,8 @@ const char* frnn_status_string(int status) {
 }
 
 size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max) {
-    if (n_total < 0 || n_events < 1 || dim != kDim || k_max < 1 || n_total > 0x7fffffffll) return 0;
-    return make_layout(n_total, n_events, choose_grid(n_total, n_events)).total;
+    if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDim || k_max < 1 || n_total > 0x7fffffffll) return 0;
+    return make_layout(n_total, n_events, choose_grid(n_total, n_events, dim)).total;
 }
 
 int frnn_set_grid(int grid_dims, int grid_bits) {
@@ -393,7 +395,7 @@ int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
     int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
     if (rc != FRNN_OK) return rc;
     if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
-    Call c{points, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
+    Call c{points, dim, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
     if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
     return run_call(c, static_cast<cudaStream_t>(cuda_stream));
 }
@@ -406,7 +408,7 @@ int frnn_build_dense_ex(const float* points, int64_t n, int dim, float r, int k_
     if (rc != FRNN_OK) return rc;
     if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
     if (n > 65535ll * kDenseTile) return FRNN_ERR_UNSUPPORTED;                 // grid.y limit (8.3 M rows)
-    Call c{points, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
+    Call c{points, dim, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
     c.dense = true;
     if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
     return run_call(c, static_cast<cudaStream_t>(cuda_stream));
@@ -422,7 +424,7 @@ int frnn_build_batched(const float* points, const int64_t* event_offsets, int n_
     int rc = check_common(points, event_offsets[n_events], dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
     if (rc != FRNN_OK) return rc;
     if (!out_edge_offsets || !out_status) return FRNN_ERR_INVALID_ARG;
-    Call c{points, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets, out_status, out_row_ptr,
+    Call c{points, dim, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets, out_status, out_row_ptr,
            workspace, 0, 0, std::vector<int64_t>(event_offsets, event_offsets + n_events + 1)};
     if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
     return run_call(c, static_cast<cudaStream_t>(cuda_stream));
@@ -460,7 +462,7 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     if ((rc = ensure_stream()) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.ws, &g_cache.ws_bytes, need)) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.misc, &misc_have, 64)) != FRNN_OK) return rc;
-    if ((rc = ensure(&g_cache.pts, &g_cache.pts_bytes, static_cast<size_t>(n > 0 ? n : 1) * 32)) != FRNN_OK) return rc;
+    if ((rc = ensure(&g_cache.pts, &g_cache.pts_bytes, static_cast<size_t>(n > 0 ? n : 1) * 32)) != FRNN_OK) return rc;   // room for 8 floats per row whatever dim is
     if (g_cache.edge_cap < static_cast<size_t>(edge_capacity) || !g_cache.edges) {
         if ((rc = ensure(&g_cache.edges, &edge_bytes, static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1) * 12)) != FRNN_OK) return rc;
         g_cache.edge_cap = static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1);
@@ -471,7 +473,7 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     float* d_d2 = reinterpret_cast<float*>(d_dst + g_cache.edge_cap);
     int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
     int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
-    if (n > 0) CK(cudaMemcpyAsync(g_cache.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, st));
+    if (n > 0) CK(cudaMemcpyAsync(g_cache.pts, points, static_cast<size_t>(n) * dim * 4, cudaMemcpyHostToDevice, st));
     rc = frnn_build_ex(static_cast<const float*>(g_cache.pts), n, dim, r, k_max, d_src, d_dst, d_d2, edge_capacity, d_count, d_status,
                        nullptr, g_cache.ws, g_cache.ws_bytes, st);
     if (rc != FRNN_OK) return rc;

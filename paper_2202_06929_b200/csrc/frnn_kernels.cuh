@@ -102,6 +102,22 @@ __device__ __forceinline__ void store_row(float4* p, const float4& a, const floa
                  :: "l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w) : "memory");
 }
 
+// A point of the caller's array as an 8-float row.  dim == 8: one 256-bit load (rows are 32-byte aligned).  dim < 8
+// (SURVEY.md 8(f) f3): the row is read float by float and padded with zeros: every padded term of the R3 chain is
+// t = 0 - 0 = +0, fma(+0, +0, acc) = acc, so d2 over 8 terms equals d2 over dim terms bit for bit.
+__device__ __forceinline__ void load_point(const float* __restrict__ pts, int64_t i, int dim, float4& a, float4& b) {
+    if (dim == kDim) {
+        load_row_nc(reinterpret_cast<const float4*>(pts) + 2 * i, a, b);
+    } else {
+        float x[kDim];
+        const float* p = pts + i * dim;
+#pragma unroll
+        for (int d = 0; d < kDim; ++d) x[d] = d < dim ? p[d] : 0.0f;
+        a = make_float4(x[0], x[1], x[2], x[3]);
+        b = make_float4(x[4], x[5], x[6], x[7]);
+    }
+}
+
 // Optional in-graph timeline (frnn_set_profiling(2)): every kernel leaves min(start) and max(end) of the
 // %globaltimer readings of thread 0 of its blocks (every 16th block for the start) in stamps[2*phase], stamps[2*phase+1] (start stored complemented so that
 // one atomicMax serves both; the buffer is zeroed with the rest of the workspace head).  stamps == NULL
@@ -142,7 +158,7 @@ __global__ void set_offsets_kernel(OffsetChunk c, int64_t* __restrict__ ev_off) 
 // which makes the later scatter a pure function of (cell_start, rank): no second atomic pass.
 // ------------------------------------------------------------------------------------------------
 template <int G>
-__global__ void __launch_bounds__(256) bin_kernel(const float4* __restrict__ pts, int64_t n_total,
+__global__ void __launch_bounds__(256) bin_kernel(const float* __restrict__ pts, int dim, int64_t n_total,
                                                   const int64_t* __restrict__ ev_off, int n_events,
                                                   float inv_cell, int bits,
                                                   uint32_t* __restrict__ cell_count,
@@ -151,9 +167,8 @@ __global__ void __launch_bounds__(256) bin_kernel(const float4* __restrict__ pts
     stamp_begin(stamps, 0);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < n_total) {
-        const float4 a = pts[2 * i];
-        float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (G > 4) b = pts[2 * i + 1];
+        float4 a, b;
+        load_point(pts, i, dim, a, b);
         const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
         const uint32_t lin = cell_of_point<G>(a, b, ev, inv_cell, bits);
         pcell[i] = lin;
@@ -167,7 +182,7 @@ __global__ void __launch_bounds__(256) bin_kernel(const float4* __restrict__ pts
 // result does not depend on it because every row is ordered by dst at the end.
 // ------------------------------------------------------------------------------------------------
 template <int G>
-__global__ void __launch_bounds__(256) scatter_kernel(const float4* __restrict__ pts, int64_t n_total, int bits, float inv_cell,
+__global__ void __launch_bounds__(256) scatter_kernel(const float* __restrict__ pts, int dim, int64_t n_total, int bits, float inv_cell,
                                                       const uint32_t* __restrict__ cell_start,
                                                       const uint32_t* __restrict__ pcell,
                                                       const uint32_t* __restrict__ prank,
@@ -178,7 +193,7 @@ __global__ void __launch_bounds__(256) scatter_kernel(const float4* __restrict__
     if (i < n_total) {
         const uint32_t s = cell_start[padded(pcell[i], bits)] + prank[i];
         float4 a, b;
-        load_row_nc(pts + 2 * i, a, b);
+        load_point(pts, i, dim, a, b);
         store_row(spts + 2 * static_cast<int64_t>(s), a, b);      // one 32-byte sector, one transaction
         sidx[s] = static_cast<int32_t>(i);
         skey[s] = key_of_point<G>(a, b, inv_cell);
@@ -661,7 +676,8 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
 // ------------------------------------------------------------------------------------------------
 constexpr int kDenseTile = 128;
 struct DenseArgs {
-    const float4* pts;
+    const float* pts;
+    int dim;
     uint32_t* cnt;
     int2* hits;
     unsigned long long* tile_deg;
@@ -679,9 +695,9 @@ __global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
     const int64_t i = static_cast<int64_t>(I) * kDenseTile + tid;
     const int64_t jr = static_cast<int64_t>(J) * kDenseTile + tid;
     float4 qa = make_float4(0.f, 0.f, 0.f, 0.f), qb = qa;
-    if (i < a.n) load_row_nc(a.pts + 2 * i, qa, qb);
+    if (i < a.n) load_point(a.pts, i, a.dim, qa, qb);
     float4 ca = make_float4(__int_as_float(0x7f800000), 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (jr < a.n) load_row_nc(a.pts + 2 * jr, ca, cb);                 // rows beyond the event: +inf, never within r
+    if (jr < a.n) load_point(a.pts, jr, a.dim, ca, cb);                 // rows beyond the event: +inf, never within r
     s_c[tid][0] = ca; s_c[tid][1] = cb;
     __syncthreads();
     if (i >= a.n) return;
@@ -791,7 +807,8 @@ __device__ __forceinline__ void warp_sort_rows(int32_t* dst, float* d2, int64_t 
 }
 
 struct EmitArgs {
-    const float4* pts;            // original points (to recompute the cell of a big row)
+    const float* pts;             // original points (to recompute the cell of a big row), n x dim
+    int dim;
     const float4* spts;
     const int32_t* sidx;
     const uint32_t* cell_start;
@@ -829,7 +846,7 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
             for (int64_t j0 = row_ev; j0 < ev_end; j0 += 32) {
                 const int64_t j = j0 + lane;
                 float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (j < ev_end) { ca = a.pts[2 * j]; cb = a.pts[2 * j + 1]; }
+                if (j < ev_end) load_point(a.pts, j, a.dim, ca, cb);
                 const float d2 = d2_pinned(qa, qb, ca, cb);
                 g(j < ev_end && d2 <= a.r2 && j != row, static_cast<int32_t>(j), d2);
             }
@@ -1012,7 +1029,8 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
             const int64_t row_rp = __shfl_sync(kFull, rp, bl);
             const int64_t row_ev = __shfl_sync(kFull, ev_base, bl);
             const uint32_t row_cnt = __shfl_sync(kFull, c, bl);
-            const float4 qa = a.pts[2 * row], qb = a.pts[2 * row + 1];
+            float4 qa, qb;
+            load_point(a.pts, row, a.dim, qa, qb);
             uint32_t ev = 0;
             if (a.ev_off) ev = static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, row));
             const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, a.bits);

@@ -217,7 +217,8 @@ def test_host_detectable_errors(F):
     assert call(**args(k=0)) == F.FRNN_ERR_INVALID_ARG
     assert call(**args(p=None)) == F.FRNN_ERR_INVALID_ARG
     assert call(**args(p=pts.data_ptr() + 16)) == F.FRNN_ERR_INVALID_ARG      # rows must be 32-byte aligned
-    assert call(**args(dim=3)) == F.FRNN_ERR_UNSUPPORTED
+    assert call(**args(dim=9)) == F.FRNN_ERR_UNSUPPORTED
+    assert call(**args(dim=0)) == F.FRNN_ERR_UNSUPPORTED
     assert call(**args(), wsbytes=128) == F.FRNN_ERR_WORKSPACE
     torch.cuda.synchronize()
     assert "capacity" in F.frnn_status_string(F.FRNN_ERR_CAPACITY)
@@ -372,3 +373,31 @@ def test_non_finite_coordinates_cannot_fault(F):
         keep_e = ~(bad[exp.src] | bad[exp.dst])
         keep_g = ~(bad[s] | bad[d])
         assert np.array_equal(s[keep_g], exp.src[keep_e]) and np.array_equal(d[keep_g], exp.dst[keep_e])
+
+
+# ---------------------------------------------------------------- embedding dimensions below 8
+@pytest.mark.parametrize("dim", [1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("entry", ["frnn_build_ex", "frnn_build_dense_ex"])
+def test_lower_dimensional_points(F, dim, entry):
+    """Rows of dim < 8 floats (unaligned stride): padded with zeros internally, d2 over dim terms bit for bit."""
+    n = 3000
+    x = events.uniform_points(n, dim, -1.0, 1.0, 40 + dim)
+    r = {1: 0.002, 2: 0.03, 3: 0.1, 4: 0.2, 5: 0.3, 6: 0.4, 7: 0.5}[dim]
+    for k in (3, 64):
+        exp = oracle.frnn(x, r, k, oracle.BRUTE)
+        assert exp.count > 500
+        res = getattr(F, entry)(torch.from_numpy(x).cuda(), r, k)
+        torch.cuda.synchronize()
+        res.check()
+        s_, d_, q_ = (t.cpu().numpy() for t in res.trimmed())
+        assert_same(Got(s_, d_, q_), exp, r, f"dim={dim} K={k}")
+
+
+@pytest.mark.parametrize("L,D,fac", [(4, 4, 1.0), (4, 4, 1.5), (4, 4, 1.8), (5, 3, 1.0), (5, 3, 1.5), (5, 3, 1.8)])
+def test_lattice_closed_form_low_dim(F, L, D, fac):
+    from tests.test_oracle_pins import lattice_closed_form
+    x = events.lattice(L, D, 0.125)
+    r = float(np.float32(fac * 0.125))
+    got, _ = run_gpu(F, x, r, 1024)
+    assert len(got.src) == lattice_closed_form(L, D, fac)
+    assert_same(got, oracle.frnn(x, r, 1024, oracle.BRUTE), r, f"lattice L={L} D={D} fac={fac}")
