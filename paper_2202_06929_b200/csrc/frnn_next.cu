@@ -58,13 +58,12 @@ __global__ void __launch_bounds__(256) cc_init_kernel(int32_t* __restrict__ pare
     if (i == 0 && n_components) *n_components = 0;
 }
 
-__device__ __forceinline__ int32_t cc_find(int32_t* parent, int32_t x) {
-    // path halving; the racing writes only ever replace a pointer by one of its ancestors
-    volatile int32_t* p = parent;
-    int32_t px = p[x];
+// find with path halving, starting from x whose parent px has already been loaded (L2-coherent loads: other blocks
+// update the array concurrently); the racing writes only ever replace a pointer by one of its ancestors
+__device__ __forceinline__ int32_t cc_find(int32_t* parent, int32_t x, int32_t px) {
     while (px != x) {
-        const int32_t gp = p[px];
-        if (gp != px) p[x] = gp;
+        const int32_t gp = __ldcg(parent + px);
+        if (gp != px) __stcg(parent + x, gp);
         x = px;
         px = gp;
     }
@@ -79,18 +78,23 @@ __global__ void __launch_bounds__(256) cc_hook_kernel(int32_t* __restrict__ pare
     if (edge_count) { const int64_t c = *edge_count; e_end = c < e_end ? c : e_end; }
     for (int64_t e = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; e < e_end;
          e += static_cast<int64_t>(gridDim.x) * blockDim.x) {
-        if (score && !(score[e] >= threshold)) continue;
         int32_t u = src[e], v = dst[e];
+        const float sc = score ? score[e] : 0.0f;                   // the three loads of the edge travel together
+        if (score && !(sc >= threshold)) continue;
         if (u < 0 || v < 0 || u >= n || v >= n || u == v) continue;
+        int32_t pu = __ldcg(parent + u), pv = __ldcg(parent + v);   // both parents in flight
+        if (pu == pv) continue;                                     // already in one tree (the usual case once a track is linked)
         while (true) {
-            u = cc_find(parent, u);
-            v = cc_find(parent, v);
+            u = cc_find(parent, u, pu);
+            v = cc_find(parent, v, pv);
             if (u == v) break;
             if (u < v) { const int32_t t = u; u = v; v = t; }      // u is the larger root
             const int32_t old = atomicCAS(&parent[u], u, v);       // link it under the smaller one
             if (old == u) break;
-            u = old;                                               // somebody linked u first: start again from there
+            pu = old;                                              // somebody linked u first: go on from there
+            pv = v;                                                // v was a root a moment ago
         }
+
     }
 }
 
@@ -105,9 +109,14 @@ __global__ void __launch_bounds__(256) cc_flatten_kernel(int32_t* __restrict__ p
         p[i] = r;
         root = r == static_cast<int32_t>(i);
     }
-    if (n_components) {
+    if (n_components) {                                            // one atomic per block
+        __shared__ int s_roots;
+        if (threadIdx.x == 0) s_roots = 0;
+        __syncthreads();
         const unsigned m = __ballot_sync(0xffffffffu, root);
-        if ((threadIdx.x & 31) == 0 && m) atomicAdd(n_components, __popc(m));
+        if ((threadIdx.x & 31) == 0 && m) atomicAdd(&s_roots, __popc(m));
+        __syncthreads();
+        if (threadIdx.x == 0 && s_roots) atomicAdd(n_components, s_roots);
     }
 }
 
