@@ -194,12 +194,12 @@ const char* frnn_phase_name(int phase);
  * In-graph timeline.  frnn_set_profiling(2) (instead of 1) keeps the CUDA-graph replay and makes every
  * kernel of later calls leave the earliest start and the latest end of its warps (%globaltimer) in the
  * call's workspace; frnn_get_timeline synchronises nothing itself (the caller waits for the call first),
- * copies the stamps of the LAST call that used `workspace` (a device pointer; n_total / n_events as in
+ * copies the stamps of the LAST call that used `workspace` (a device pointer; n_total / n_events / dim as in
  * that call) and writes, per kernel (bin, scan_cells, scatter, search, emit), begin and end in
  * microseconds relative to the start of the first kernel.  Returns the number of kernels written or a
  * negative status.  Unlike mode 1 this does not perturb the launch sequence.
  */
-int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events,
+int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, int dim,
                       double* begin_us /* HOST */, double* end_us /* HOST */, int max_phases);
 const char* frnn_timeline_name(int phase);
 

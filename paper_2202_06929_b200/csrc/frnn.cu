@@ -630,9 +630,9 @@ int frnn_get_profile(float* phase_ms, int max_phases) {
     return n;
 }
 
-int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, double* begin_us, double* end_us, int max_phases) {
-    if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1) return FRNN_ERR_INVALID_ARG;
-    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events));
+int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, int dim, double* begin_us, double* end_us, int max_phases) {
+    if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1 || dim < 1 || dim > kDim) return FRNN_ERR_INVALID_ARG;
+    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events, dim));
     unsigned long long h[2 * kTimelinePhases];
     if (cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess)
         return FRNN_ERR_CUDA;

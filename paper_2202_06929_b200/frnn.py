@@ -49,7 +49,7 @@ _SIGNATURES = {
     "frnn_set_profiling": (_c.c_int, [_c.c_int]),
     "frnn_get_profile": (_c.c_int, [_c.POINTER(_c.c_float), _c.c_int]),
     "frnn_phase_name": (_c.c_char_p, [_c.c_int]),
-    "frnn_get_timeline": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_double), _c.c_int]),
+    "frnn_get_timeline": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_int, _c.POINTER(_c.c_double), _c.POINTER(_c.c_double), _c.c_int]),
     "frnn_timeline_name": (_c.c_char_p, [_c.c_int]),
     "frnn_gather_edge_rows": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_void_p, _c.c_void_p, _c.c_void_p,
                                          _c.c_int64, _c.c_int64, _c.c_int64, _c.c_void_p, _c.c_void_p]),
@@ -132,11 +132,11 @@ def frnn_set_profiling(enabled) -> None:
     _check(lib().frnn_set_profiling(int(enabled)), "frnn_set_profiling")
 
 
-def frnn_get_timeline(workspace: torch.Tensor, n_total: int, n_events: int = 1) -> dict[str, tuple[float, float]]:
+def frnn_get_timeline(workspace: torch.Tensor, n_total: int, n_events: int = 1, dim: int = 8) -> dict[str, tuple[float, float]]:
     """(begin_us, end_us) per kernel of the last call on ``workspace`` made in profiling mode 2
     (the caller synchronises first)."""
     b, e = (_c.c_double * 8)(), (_c.c_double * 8)()
-    n = lib().frnn_get_timeline(_ptr(workspace), int(n_total), int(n_events), b, e, 8)
+    n = lib().frnn_get_timeline(_ptr(workspace), int(n_total), int(n_events), int(dim), b, e, 8)
     if n < 0:
         raise FrnnError(n, "frnn_get_timeline")
     return {lib().frnn_timeline_name(i).decode(): (float(b[i]), float(e[i])) for i in range(n)}
