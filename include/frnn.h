@@ -21,10 +21,11 @@
  *   - Every pointer is a DEVICE pointer owned by the caller unless marked HOST.  The library never
  *     allocates or frees caller-visible memory.  frnn_build_ex / frnn_build_batched only enqueue
  *     work on `cuda_stream` (a cudaStream_t; NULL = legacy default stream) and never synchronise.
- *   - points: row-major n x dim fp32, 1 <= dim <= 8 (FRNN_ERR_UNSUPPORTED otherwise).  dim == 8 is the fast path:
- *     base 32-byte aligned (a row moves as one 256-bit transaction; FRNN_ERR_INVALID_ARG otherwise).  dim < 8
- *     (SURVEY.md 8(f) f3): rows are read float by float and padded with zeros internally, which leaves every d2
- *     bit-identical to the dim-term chain; the grid then bins at most dim coordinates.  Finite values (non-finite coordinates
+ *   - points: row-major n x dim fp32, 1 <= dim <= 16 (FRNN_ERR_UNSUPPORTED otherwise).  dim == 8 is the fast path:
+ *     base 32-byte aligned (a row moves as one 256-bit transaction; FRNN_ERR_INVALID_ARG otherwise).  Other dims
+ *     (SURVEY.md 8(f) f3): rows are read float by float and padded with zeros internally -- to 8 floats, or to 16 in
+ *     two internal rows when dim > 8 -- which leaves every d2 bit-identical to the dim-term chain; the grid bins at
+ *     most dim coordinates and never a coordinate beyond the 8th.  Finite values (non-finite coordinates
  *     are a precondition violation; they can never cause an out-of-bounds access).
  *   - src/dst are int32 row indices (local to the event in the batched call); counts and offsets
  *     are int64.  Edges of one call are sorted by (src, dst) ascending and free of duplicates.
@@ -51,7 +52,7 @@ extern "C" {
 typedef enum {
     FRNN_OK = 0,
     FRNN_ERR_INVALID_ARG = -1,  /* null or misaligned pointer, n < 0, r < 0 or not finite, k_max < 1, bad offsets */
-    FRNN_ERR_UNSUPPORTED = -2,  /* dim outside 1..8 (host-buffer and edge-row calls: dim != 8), more than 2^31-1 rows */
+    FRNN_ERR_UNSUPPORTED = -2,  /* dim outside 1..16 (host pipeline and edge-row calls: dim != 8), more than 2^31-1 rows */
     FRNN_ERR_CAPACITY = -3,     /* device-detected: more edges than edge_capacity */
     FRNN_ERR_WORKSPACE = -4,    /* workspace_bytes < frnn_workspace_bytes(...) */
     FRNN_ERR_CUDA = -5          /* a CUDA runtime call failed (or no device) */

@@ -65,11 +65,11 @@ struct Layout {
     int rows_per_block;
     int64_t scan_blocks;
     size_t off_cells, off_tiles, off_counters, zero_bytes;
-    size_t off_pcell, off_prank, off_spts, off_sidx, off_skey, off_cnt, off_evoff, off_hits, off_tprefix;
+    size_t off_pcell, off_prank, off_spts, off_spts_hi, off_sidx, off_skey, off_cnt, off_evoff, off_hits, off_tprefix;
     size_t total;
 };
 
-Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
+Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim = kDim) {
     Layout L;
     L.n_cells = static_cast<int64_t>(n_events) << (g.dims * g.bits);
     const int64_t row_len = (1ll << g.bits) + 1;
@@ -89,6 +89,7 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g) {
     L.off_pcell = o;  o = align_up(o + n * 4);
     L.off_prank = o;  o = align_up(o + n * 4);
     L.off_spts = o;   o = align_up(o + n * 32);
+    L.off_spts_hi = o; if (dim > kDim) o = align_up(o + n * 32);      // coordinates 8..15 of the cell-ordered copy
     L.off_sidx = o;   o = align_up(o + n * 4);
     L.off_skey = o;   o = align_up(o + n * 4);
     L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
@@ -115,7 +116,7 @@ int check_common(const float* points, int64_t n, int dim, float r, int k_max, co
     if (n < 0 || k_max < 1 || capacity < 0) return FRNN_ERR_INVALID_ARG;
     if (!(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
     if (n > 0 && !points) return FRNN_ERR_INVALID_ARG;
-    if (dim < 1 || dim > kDim) return FRNN_ERR_UNSUPPORTED;
+    if (dim < 1 || dim > kDimMax) return FRNN_ERR_UNSUPPORTED;
     if (reinterpret_cast<uintptr_t>(points) % (dim == kDim ? 32 : 4)) return FRNN_ERR_INVALID_ARG;   // 8-float rows move as 256-bit transactions
     if (capacity > 0 && (!out_src || !out_dst || !out_d2)) return FRNN_ERR_INVALID_ARG;
     if (n > 0x7fffffffll) return FRNN_ERR_UNSUPPORTED;
@@ -160,6 +161,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
+    float4* spts_hi = c.dim > kDim ? reinterpret_cast<float4*>(ws + L.off_spts_hi) : nullptr;
     int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
     uint32_t* skey = reinterpret_cast<uint32_t*>(ws + L.off_skey);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
@@ -179,10 +181,11 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
         da.pts = pts; da.dim = c.dim; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = static_cast<uint32_t>(L.emit_tiles);
         da.n = n_total; da.r2 = r2; da.k_max = static_cast<uint32_t>(c.k_max);
         const unsigned T = static_cast<unsigned>((n_total + kDenseTile - 1) / kDenseTile);
-        dense_search_kernel<<<dim3(T, T), kDenseTile, 0, st>>>(da);
+        if (c.dim > kDim) dense_search_kernel<true><<<dim3(T, T), kDenseTile, 0, st>>>(da);
+        else              dense_search_kernel<false><<<dim3(T, T), kDenseTile, 0, st>>>(da);
         ++t_launches; CK(cudaGetLastError());
         EmitArgs ea;
-        ea.pts = pts; ea.dim = c.dim; ea.spts = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.cnt = cnt; ea.hits = hits; ea.ev_off = nullptr;
+        ea.pts = pts; ea.dim = c.dim; ea.spts = nullptr; ea.spts_hi = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.cnt = cnt; ea.hits = hits; ea.ev_off = nullptr;
         ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = 1; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
         ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
         ea.out_edge_offsets = nullptr; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
@@ -220,21 +223,22 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor, stamps);
     ++t_launches; CK(cudaGetLastError());
     mark(2, st);
-    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, stamps)));
+    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, spts_hi, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(3, st);
 
     SearchArgs sa;
-    sa.spts = spts; sa.sidx = sidx; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
+    sa.spts = spts; sa.spts_hi = spts_hi; sa.sidx = sidx; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
     sa.tile_deg = tile_deg; sa.n_tiles = static_cast<uint32_t>(L.emit_tiles); sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
     sa.inv_cell = inv_cell; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
     const unsigned search_blocks = static_cast<unsigned>((n_total + kSearchThreads - 1) / kSearchThreads);
-    FRNN_DISPATCH_G(G, (search_kernel<GG><<<search_blocks, kSearchThreads, 0, st>>>(sa)));
+    if (spts_hi) { FRNN_DISPATCH_G(G, (search_kernel<GG, true><<<search_blocks, kSearchThreads, 0, st>>>(sa))); }
+    else         { FRNN_DISPATCH_G(G, (search_kernel<GG, false><<<search_blocks, kSearchThreads, 0, st>>>(sa))); }
     ++t_launches; CK(cudaGetLastError());
     mark(4, st);
 
     EmitArgs ea;
-    ea.pts = pts; ea.dim = c.dim; ea.spts = spts; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
+    ea.pts = pts; ea.dim = c.dim; ea.spts = spts; ea.spts_hi = spts_hi; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
     ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
@@ -269,7 +273,7 @@ int run_call(const Call& c, cudaStream_t st) {
         CK(cudaMemsetAsync(c.out_status, 0, 4, st)); ++t_launches;
         return FRNN_OK;
     }
-    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits});
+    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits}, c.dim);
     bool graph_ok = g_use_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
     if (graph_ok) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
@@ -318,7 +322,7 @@ int prepare(Call& c, size_t workspace_bytes) {
     c.grid_bits = g.bits;
     c.timeline = g_timeline;
     if (n_total == 0) return FRNN_OK;
-    const Layout L = make_layout(n_total, c.n_events, g);
+    const Layout L = make_layout(n_total, c.n_events, g, c.dim);
     if (!c.workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
     if (reinterpret_cast<uintptr_t>(c.workspace) % kAlign) return FRNN_ERR_INVALID_ARG;
     return FRNN_OK;
@@ -357,7 +361,7 @@ const char* frnn_status_string(int status) {
     switch (status) {
         case FRNN_OK: return "ok";
         case FRNN_ERR_INVALID_ARG: return "invalid argument";
-        case FRNN_ERR_UNSUPPORTED: return "unsupported (dim outside 1..8 or too many rows)";
+        case FRNN_ERR_UNSUPPORTED: return "unsupported (dim outside 1..16 or too many rows)";
         case FRNN_ERR_CAPACITY: return "edge capacity exceeded";
         case FRNN_ERR_WORKSPACE: return "workspace too small";
         case FRNN_ERR_CUDA: return "CUDA error";
@@ -366,8 +370,8 @@ const char* frnn_status_string(int status) {
 }
 
 size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max) {
-    if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDim || k_max < 1 || n_total > 0x7fffffffll) return 0;
-    return make_layout(n_total, n_events, choose_grid(n_total, n_events, dim)).total;
+    if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDimMax || k_max < 1 || n_total > 0x7fffffffll) return 0;
+    return make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim).total;
 }
 
 int frnn_set_grid(int grid_dims, int grid_bits) {
@@ -462,7 +466,7 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     if ((rc = ensure_stream()) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.ws, &g_cache.ws_bytes, need)) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.misc, &misc_have, 64)) != FRNN_OK) return rc;
-    if ((rc = ensure(&g_cache.pts, &g_cache.pts_bytes, static_cast<size_t>(n > 0 ? n : 1) * 32)) != FRNN_OK) return rc;   // room for 8 floats per row whatever dim is
+    if ((rc = ensure(&g_cache.pts, &g_cache.pts_bytes, static_cast<size_t>(n > 0 ? n : 1) * 64)) != FRNN_OK) return rc;   // room for 16 floats per row whatever dim is
     if (g_cache.edge_cap < static_cast<size_t>(edge_capacity) || !g_cache.edges) {
         if ((rc = ensure(&g_cache.edges, &edge_bytes, static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1) * 12)) != FRNN_OK) return rc;
         g_cache.edge_cap = static_cast<size_t>(edge_capacity > 0 ? edge_capacity : 1);
@@ -631,8 +635,8 @@ int frnn_get_profile(float* phase_ms, int max_phases) {
 }
 
 int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, int dim, double* begin_us, double* end_us, int max_phases) {
-    if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1 || dim < 1 || dim > kDim) return FRNN_ERR_INVALID_ARG;
-    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events, dim));
+    if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1 || dim < 1 || dim > kDimMax) return FRNN_ERR_INVALID_ARG;
+    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim);
     unsigned long long h[2 * kTimelinePhases];
     if (cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess)
         return FRNN_ERR_CUDA;

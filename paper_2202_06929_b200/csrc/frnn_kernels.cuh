@@ -18,7 +18,8 @@
 
 namespace frnn {
 
-constexpr int kDim = 8;
+constexpr int kDim = 8;                 // floats of an internal row (and of the fast path's input rows)
+constexpr int kDimMax = 16;            // dim 9..16: a second internal row holds coordinates 8..15 (zero padded)
 constexpr unsigned kFull = 0xffffffffu;
 
 // ------------------------------------------------------------------------------------------------
@@ -102,9 +103,10 @@ __device__ __forceinline__ void store_row(float4* p, const float4& a, const floa
                  :: "l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w), "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w) : "memory");
 }
 
-// A point of the caller's array as an 8-float row.  dim == 8: one 256-bit load (rows are 32-byte aligned).  dim < 8
-// (SURVEY.md 8(f) f3): the row is read float by float and padded with zeros: every padded term of the R3 chain is
-// t = 0 - 0 = +0, fma(+0, +0, acc) = acc, so d2 over 8 terms equals d2 over dim terms bit for bit.
+// A point of the caller's array as an 8-float row (coordinates 0..7).  dim == 8: one 256-bit load (rows are 32-byte
+// aligned).  Other dims: the row is read float by float and padded with zeros: every padded term
+// of the R3 chain is t = 0 - 0 = +0, fma(+0, +0, acc) = acc, so d2 over the padded row equals d2 over dim terms bit
+// for bit.  load_point_hi: coordinates 8..15 of a point with dim > 8, same padding.
 __device__ __forceinline__ void load_point(const float* __restrict__ pts, int64_t i, int dim, float4& a, float4& b) {
     if (dim == kDim) {
         load_row_nc(reinterpret_cast<const float4*>(pts) + 2 * i, a, b);
@@ -116,6 +118,14 @@ __device__ __forceinline__ void load_point(const float* __restrict__ pts, int64_
         a = make_float4(x[0], x[1], x[2], x[3]);
         b = make_float4(x[4], x[5], x[6], x[7]);
     }
+}
+__device__ __forceinline__ void load_point_hi(const float* __restrict__ pts, int64_t i, int dim, float4& c, float4& d) {
+    float x[kDim];
+    const float* p = pts + i * dim + kDim;
+#pragma unroll
+    for (int k = 0; k < kDim; ++k) x[k] = kDim + k < dim ? p[k] : 0.0f;
+    c = make_float4(x[0], x[1], x[2], x[3]);
+    d = make_float4(x[4], x[5], x[6], x[7]);
 }
 
 // Optional in-graph timeline (frnn_set_profiling(2)): every kernel leaves min(start) and max(end) of the
@@ -132,6 +142,20 @@ __device__ __forceinline__ void stamp_begin(unsigned long long* stamps, int phas
 }
 __device__ __forceinline__ void stamp_end(unsigned long long* stamps, int phase) {
     if (stamps && threadIdx.x == 0) atomicMax(&stamps[2 * phase + 1], global_ns());
+}
+
+// dims 8..15 of a pair: the chain simply goes on (R3: one fp32 chain over d = 0..dim-1 in index order)
+__device__ __forceinline__ float d2_continue(float acc, const float4& qc, const float4& qd, const float4& cc, const float4& cd) {
+    float t;
+    t = __fsub_rn(qc.x, cc.x); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qc.y, cc.y); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qc.z, cc.z); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qc.w, cc.w); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qd.x, cd.x); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qd.y, cd.y); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qd.z, cd.z); acc = __fmaf_rn(t, t, acc);
+    t = __fsub_rn(qd.w, cd.w); acc = __fmaf_rn(t, t, acc);
+    return acc;
 }
 
 __device__ __forceinline__ int event_of_row(const int64_t* __restrict__ ev_off, int n_events, int64_t row) {
@@ -187,7 +211,8 @@ __global__ void __launch_bounds__(256) scatter_kernel(const float* __restrict__ 
                                                       const uint32_t* __restrict__ pcell,
                                                       const uint32_t* __restrict__ prank,
                                                       float4* __restrict__ spts, int32_t* __restrict__ sidx,
-                                                      uint32_t* __restrict__ skey, unsigned long long* stamps) {
+                                                      uint32_t* __restrict__ skey, float4* __restrict__ spts_hi,
+                                                      unsigned long long* stamps) {
     stamp_begin(stamps, 2);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < n_total) {
@@ -197,6 +222,11 @@ __global__ void __launch_bounds__(256) scatter_kernel(const float* __restrict__ 
         store_row(spts + 2 * static_cast<int64_t>(s), a, b);      // one 32-byte sector, one transaction
         sidx[s] = static_cast<int32_t>(i);
         skey[s] = key_of_point<G>(a, b, inv_cell);
+        if (spts_hi) {                                             // dim > 8: coordinates 8..15 travel in a second row
+            float4 c, d;
+            load_point_hi(pts, i, dim, c, d);
+            store_row(spts_hi + 2 * static_cast<int64_t>(s), c, d);
+        }
     }
     stamp_end(stamps, 2);
 }
@@ -407,6 +437,7 @@ constexpr int kDegSlices = FRNN_DEG_SLICES;   // copies of every per-tile degree
 
 struct SearchArgs {
     const float4* spts;
+    const float4* spts_hi;        // coordinates 8..15 of the slots (dim > 8), else NULL
     const int32_t* sidx;          // slot -> global row index
     const uint32_t* skey;         // slot -> filter key
     const uint32_t* cell_start;
@@ -454,7 +485,7 @@ __device__ __forceinline__ void leftover_push(uint32_t& laddr, uint32_t j0, uint
         : "memory");
 }
 
-template <int G>
+template <int G, bool HI>
 __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search_kernel(SearchArgs a) {
     constexpr int NU = G >= 2 ? 3 : 1;                    // unrolled offsets of coordinate G-2
     constexpr int NB = pow3(G >= 2 ? G - 2 : 0);          // sub-batches: offsets of coordinates 0..G-3 (dim 0 most significant)
@@ -509,19 +540,29 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
         for (int i = 0; i < qn; i += kWide) {
             float4 ca[kWide], cb[kWide];
             int32_t cj[kWide];
+            uint32_t js[kWide];
             bool ok[kWide];
 #pragma unroll
             for (int v = 0; v < kWide; ++v) {
                 ok[v] = i + v < qn;
-                const uint32_t j = ok[v] ? s_queue[i + v][tid] : s;      // padding: my own row (a valid address, masked below)
-                load_row_nc(a.spts + 2 * static_cast<int64_t>(j), ca[v], cb[v]);
-                cj[v] = a.sidx[j];
+                js[v] = ok[v] ? s_queue[i + v][tid] : s;                 // padding: my own row (a valid address, masked below)
+                load_row_nc(a.spts + 2 * static_cast<int64_t>(js[v]), ca[v], cb[v]);
+                cj[v] = a.sidx[js[v]];
             }
             float d2[kWide];
+#pragma unroll
+            for (int v = 0; v < kWide; ++v) d2[v] = d2_pinned(qa, qb, ca[v], cb[v]);
+            if (HI) {                                                    // dim > 8: the chain goes on over coordinates 8..15
+                float4 qc, qd;
+                load_row_nc(a.spts_hi + 2 * s64, qc, qd);
+#pragma unroll
+                for (int v = 0; v < kWide; ++v) load_row_nc(a.spts_hi + 2 * static_cast<int64_t>(js[v]), ca[v], cb[v]);
+#pragma unroll
+                for (int v = 0; v < kWide; ++v) d2[v] = d2_continue(d2[v], qc, qd, ca[v], cb[v]);
+            }
             uint32_t nh = 0;
 #pragma unroll
             for (int v = 0; v < kWide; ++v) {
-                d2[v] = d2_pinned(qa, qb, ca[v], cb[v]);
                 ok[v] = ok[v] && d2[v] <= a.r2;
                 nh += ok[v];
             }
@@ -687,18 +728,26 @@ struct DenseArgs {
     uint32_t k_max;
 };
 
+template <bool HI>
 __global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
     const uint32_t I = blockIdx.y, J = blockIdx.x;
     if (J < I) return;
-    __shared__ float4 s_c[kDenseTile][2];
+    __shared__ float4 s_c[kDenseTile][HI ? 4 : 2];
     const int tid = threadIdx.x;
     const int64_t i = static_cast<int64_t>(I) * kDenseTile + tid;
     const int64_t jr = static_cast<int64_t>(J) * kDenseTile + tid;
-    float4 qa = make_float4(0.f, 0.f, 0.f, 0.f), qb = qa;
-    if (i < a.n) load_point(a.pts, i, a.dim, qa, qb);
-    float4 ca = make_float4(__int_as_float(0x7f800000), 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (jr < a.n) load_point(a.pts, jr, a.dim, ca, cb);                 // rows beyond the event: +inf, never within r
+    float4 qa = make_float4(0.f, 0.f, 0.f, 0.f), qb = qa, qc = qa, qd = qa;
+    if (i < a.n) {
+        load_point(a.pts, i, a.dim, qa, qb);
+        if (HI) load_point_hi(a.pts, i, a.dim, qc, qd);
+    }
+    float4 ca = make_float4(__int_as_float(0x7f800000), 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f), cc = cb, cd = cb;
+    if (jr < a.n) {                                                     // rows beyond the event: +inf, never within r
+        load_point(a.pts, jr, a.dim, ca, cb);
+        if (HI) load_point_hi(a.pts, jr, a.dim, cc, cd);
+    }
     s_c[tid][0] = ca; s_c[tid][1] = cb;
+    if (HI) { s_c[tid][2] = cc; s_c[tid][3] = cd; }
     __syncthreads();
     if (i >= a.n) return;
     unsigned long long* const my_tile_deg = a.tile_deg + static_cast<size_t>(J & (kDegSlices - 1)) * a.n_tiles;
@@ -706,7 +755,8 @@ __global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
     const int32_t row = static_cast<int32_t>(i);
 #pragma unroll 4
     for (int k = k0; k < kDenseTile; ++k) {
-        const float d2 = d2_pinned(qa, qb, s_c[k][0], s_c[k][1]);
+        float d2 = d2_pinned(qa, qb, s_c[k][0], s_c[k][1]);
+        if (HI) d2 = d2_continue(d2, qc, qd, s_c[k][2], s_c[k][3]);
         if (d2 <= a.r2) {
             const int32_t cj = static_cast<int32_t>(J * kDenseTile + k);
             const int d2b = __float_as_int(d2);
@@ -810,6 +860,7 @@ struct EmitArgs {
     const float* pts;             // original points (to recompute the cell of a big row), n x dim
     int dim;
     const float4* spts;
+    const float4* spts_hi;        // coordinates 8..15 of the slots (dim > 8), else NULL
     const int32_t* sidx;
     const uint32_t* cell_start;
     const uint32_t* cnt;
@@ -839,6 +890,9 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
                                              uint32_t cell, const float4& qa, const float4& qb, int* s_delta, int lane,
                                              int lane_delta, uint32_t lt_mask) {
     const float inf = __int_as_float(0x7f800000);
+    const bool hi = a.dim > kDim;                         // coordinates 8..15 exist: the chain goes on over them
+    float4 qc = make_float4(0.f, 0.f, 0.f, 0.f), qd = qc;
+    if (hi) load_point_hi(a.pts, row, a.dim, qc, qd);
     // visit(g): g(in_radius, j, d2) once per chunk, one candidate per lane
     auto visit = [&](auto&& g) {
         if (a.dense) {                                    // every row of the event, 32 at a time, in original order
@@ -847,7 +901,12 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
                 const int64_t j = j0 + lane;
                 float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f);
                 if (j < ev_end) load_point(a.pts, j, a.dim, ca, cb);
-                const float d2 = d2_pinned(qa, qb, ca, cb);
+                float d2 = d2_pinned(qa, qb, ca, cb);
+                if (hi) {
+                    float4 cc = make_float4(0.f, 0.f, 0.f, 0.f), cd = cc;
+                    if (j < ev_end) load_point_hi(a.pts, j, a.dim, cc, cd);
+                    d2 = d2_continue(d2, qc, qd, cc, cd);
+                }
                 g(j < ev_end && d2 <= a.r2 && j != row, static_cast<int32_t>(j), d2);
             }
             return;
@@ -860,7 +919,12 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
                 cb = a.spts[2 * static_cast<int64_t>(cslot) + 1];
                 cj = a.sidx[cslot];
             }
-            const float d2 = d2_pinned(qa, qb, ca, cb);
+            float d2 = d2_pinned(qa, qb, ca, cb);
+            if (hi) {
+                float4 cc = make_float4(0.f, 0.f, 0.f, 0.f), cd = cc;
+                if (cslot >= 0) { cc = a.spts_hi[2 * static_cast<int64_t>(cslot)]; cd = a.spts_hi[2 * static_cast<int64_t>(cslot) + 1]; }
+                d2 = d2_continue(d2, qc, qd, cc, cd);
+            }
             g(d2 <= a.r2 && cj != static_cast<int32_t>(row), cj, d2);
         });
     };

@@ -194,9 +194,10 @@ class EdgeList:
 class Workspace:
     """Reusable device scratch + output buffers for repeated calls of one shape."""
 
-    def __init__(self, n_total: int, n_events: int, k_max: int, edge_capacity: int, device=None, want_row_ptr: bool = False):
+    def __init__(self, n_total: int, n_events: int, k_max: int, edge_capacity: int, device=None, want_row_ptr: bool = False,
+                 dim: int = 8):
         device = device or torch.device("cuda", torch.cuda.current_device())
-        self.bytes = frnn_workspace_bytes(n_total, n_events, 8, k_max)
+        self.bytes = frnn_workspace_bytes(n_total, n_events, dim, k_max)
         self.buf = torch.empty(max(self.bytes, 256), dtype=torch.uint8, device=device)
         self.edge_capacity = int(edge_capacity)
         cap = max(self.edge_capacity, 1)
@@ -224,7 +225,7 @@ def frnn_build_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int
     if edge_capacity is None:
         edge_capacity = ws.edge_capacity if ws is not None else n * k_max
     if ws is None:
-        ws = Workspace(n, 1, k_max, edge_capacity, points.device, want_row_ptr)
+        ws = Workspace(n, 1, k_max, edge_capacity, points.device, want_row_ptr, dim)
     stream = stream or torch.cuda.current_stream(points.device)
     st = getattr(lib(), _entry)(_ptr(points), n, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst), _ptr(ws.d2),
                                 int(edge_capacity), _ptr(ws.count), _ptr(ws.status), _ptr(ws.row_ptr),
@@ -244,7 +245,7 @@ def frnn_build_batched(points: torch.Tensor, event_offsets, r: float, k_max: int
     if edge_capacity is None:
         edge_capacity = ws.edge_capacity if ws is not None else n * k_max
     if ws is None:
-        ws = Workspace(n, n_events, k_max, edge_capacity, points.device, want_row_ptr)
+        ws = Workspace(n, n_events, k_max, edge_capacity, points.device, want_row_ptr, dim)
     count = ws.count if ws.count.numel() == n_events + 1 else torch.zeros(n_events + 1, dtype=torch.int64, device=points.device)
     stream = stream or torch.cuda.current_stream(points.device)
     c_offs = (_c.c_int64 * (n_events + 1))(*offs)

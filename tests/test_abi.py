@@ -38,7 +38,8 @@ def test_host_only_entry_points():
     assert frnn.frnn_status_string(frnn.FRNN_OK) == "ok"
     assert "workspace" in frnn.frnn_status_string(frnn.FRNN_ERR_WORKSPACE)
     assert frnn.frnn_workspace_bytes(120000, 1, 8, 256) > 120000 * 32
-    assert frnn.frnn_workspace_bytes(120000, 1, 9, 256) == 0          # dim outside 1..8
+    assert frnn.frnn_workspace_bytes(120000, 1, 17, 256) == 0         # dim outside 1..16
+    assert frnn.frnn_workspace_bytes(120000, 1, 12, 256) == frnn.frnn_workspace_bytes(120000, 1, 8, 256) + 120000 * 32   # the second internal row
     assert 0 < frnn.frnn_workspace_bytes(120000, 1, 3, 256) < frnn.frnn_workspace_bytes(120000, 1, 8, 256)   # 3 binned coordinates: smaller table
     assert frnn.frnn_workspace_bytes(-1, 1, 8, 256) == 0
     big = frnn.frnn_workspace_bytes(16 * 120000, 16, 8, 256)

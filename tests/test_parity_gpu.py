@@ -217,7 +217,7 @@ def test_host_detectable_errors(F):
     assert call(**args(k=0)) == F.FRNN_ERR_INVALID_ARG
     assert call(**args(p=None)) == F.FRNN_ERR_INVALID_ARG
     assert call(**args(p=pts.data_ptr() + 16)) == F.FRNN_ERR_INVALID_ARG      # rows must be 32-byte aligned
-    assert call(**args(dim=9)) == F.FRNN_ERR_UNSUPPORTED
+    assert call(**args(dim=17)) == F.FRNN_ERR_UNSUPPORTED
     assert call(**args(dim=0)) == F.FRNN_ERR_UNSUPPORTED
     assert call(**args(), wsbytes=128) == F.FRNN_ERR_WORKSPACE
     torch.cuda.synchronize()
@@ -376,13 +376,14 @@ def test_non_finite_coordinates_cannot_fault(F):
 
 
 # ---------------------------------------------------------------- embedding dimensions below 8
-@pytest.mark.parametrize("dim", [1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("dim", [1, 2, 3, 4, 5, 6, 7, 9, 12, 15, 16])
 @pytest.mark.parametrize("entry", ["frnn_build_ex", "frnn_build_dense_ex"])
-def test_lower_dimensional_points(F, dim, entry):
-    """Rows of dim < 8 floats (unaligned stride): padded with zeros internally, d2 over dim terms bit for bit."""
+def test_other_dimensions(F, dim, entry):
+    """Rows of dim != 8 floats (unaligned stride): padded with zeros internally (dim > 8: a second internal row for
+    coordinates 8..15), d2 over dim terms bit for bit."""
     n = 3000
     x = events.uniform_points(n, dim, -1.0, 1.0, 40 + dim)
-    r = {1: 0.002, 2: 0.03, 3: 0.1, 4: 0.2, 5: 0.3, 6: 0.4, 7: 0.5}[dim]
+    r = {1: 0.002, 2: 0.03, 3: 0.1, 4: 0.2, 5: 0.3, 6: 0.4, 7: 0.5, 9: 0.65, 12: 1.05, 15: 1.35, 16: 1.4}[dim]
     for k in (3, 64):
         exp = oracle.frnn(x, r, k, oracle.BRUTE)
         assert exp.count > 500
@@ -401,3 +402,18 @@ def test_lattice_closed_form_low_dim(F, L, D, fac):
     got, _ = run_gpu(F, x, r, 1024)
     assert len(got.src) == lattice_closed_form(L, D, fac)
     assert_same(got, oracle.frnn(x, r, 1024, oracle.BRUTE), r, f"lattice L={L} D={D} fac={fac}")
+
+
+@pytest.mark.parametrize("dim", [12, 16])
+def test_clustered_event_in_higher_dimension(F, dim):
+    """A tracking-shaped event in a 12- or 16-dimensional embedding: tight clusters + uniform noise, K binding on some rows."""
+    rng = np.random.default_rng(dim)
+    centres = rng.uniform(-1, 1, (1500, dim))
+    sig = centres[rng.integers(0, 1500, 18000)] + rng.normal(0, 0.03, (18000, dim))
+    x = np.ascontiguousarray(np.concatenate([sig, rng.uniform(-1, 1, (2000, dim))]).astype(np.float32)[rng.permutation(20000)])
+    r = 0.03 * np.sqrt(2 * dim) * 0.9
+    for k in (256, 4):
+        exp = oracle.frnn(x, r, k, oracle.CELLS)
+        assert exp.count > 20000
+        got, _ = run_gpu(F, x, r, k, capacity=exp.count + 8)
+        assert_same(got, exp, r, f"clustered dim={dim} K={k}")
