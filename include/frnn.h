@@ -83,6 +83,23 @@ int frnn_set_grid(int grid_dims, int grid_bits);
 void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits);
 
 /*
+ * Which coordinates the grid bins and which the key filter tests (PAPER.md:69 says only that the
+ * paper's grid uses "three dimensions" of the embedding, not which).  order[0..count) lists coordinate indices in
+ * [0, 16), distinct; a call whose grid bins g coordinates bins order[0..g) and keys the next four; entries not given
+ * are filled with the unused coordinates in ascending order.  count == 0 (or order == NULL) restores the default (the
+ * first g coordinates binned, the next four keyed -- the fast path).  Process-global.  The RESULT never depends on the
+ * order: every binned or keyed coordinate is a necessary condition by itself (R8); only the amount of pruning
+ * does.  The statistics of an embedding belong to the trained model, not to the event: choose once, reuse.
+ * frnn_suggest_bin_order ranks the coordinates of a sample of `points` (DEVICE, n x dim) by the probability that two
+ * random points fall within one cell (side r) of each other along that coordinate -- the smaller, the more it prunes --
+ * writes the best eight to order[0..8) (HOST) and, if score != NULL, the 16 probabilities to score (HOST; absent
+ * coordinates: 2.0).  Synchronous (one small kernel, one device allocation, a stream synchronise).
+ */
+int frnn_set_bin_order(const int* order /* HOST */, int count);
+int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int* order /* HOST, 8 */,
+                           float* score /* HOST, 16, optional */, void* cuda_stream);
+
+/*
  * Launch mode (process-global).  1 (default): a call on a non-default stream replays a cached CUDA
  * graph of its kernels (keyed by every argument; built on first use, at most 128 kept, least
  * recently used evicted) -- about 1 us per kernel boundary instead of about 3 us per stream launch.

@@ -22,6 +22,7 @@ constexpr int64_t kPrefixTilesMin = 1024;   // above this many emit tiles the ti
 
 int g_force_dims = 0, g_force_bits = 0;
 int g_use_graph = 1;
+BinOrder g_order = {0, {0, 1, 2, 3, 4, 5, 6, 7}};   // frnn_set_bin_order
 bool g_timeline = false;                    // frnn_set_profiling(2): kernels leave %globaltimer stamps in the workspace
 constexpr int kTimelinePhases = 5;
 const char* const kTimelineNames[kTimelinePhases] = {"bin", "scan_cells", "scatter", "search", "emit"};
@@ -65,11 +66,11 @@ struct Layout {
     int rows_per_block;
     int64_t scan_blocks;
     size_t off_cells, off_tiles, off_counters, zero_bytes;
-    size_t off_pcell, off_prank, off_spts, off_spts_hi, off_sidx, off_skey, off_cnt, off_evoff, off_hits, off_tprefix;
+    size_t off_pcell, off_prank, off_spts, off_spts_hi, off_scell, off_sidx, off_skey, off_cnt, off_evoff, off_hits, off_tprefix;
     size_t total;
 };
 
-Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim = kDim) {
+Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim = kDim, bool ordered = false) {
     Layout L;
     L.n_cells = static_cast<int64_t>(n_events) << (g.dims * g.bits);
     const int64_t row_len = (1ll << g.bits) + 1;
@@ -90,6 +91,7 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim = kDim) 
     L.off_prank = o;  o = align_up(o + n * 4);
     L.off_spts = o;   o = align_up(o + n * 32);
     L.off_spts_hi = o; if (dim > kDim) o = align_up(o + n * 32);      // coordinates 8..15 of the cell-ordered copy
+    L.off_scell = o;   if (ordered) o = align_up(o + n * 4);           // slot -> cell id (only with a caller-chosen bin order)
     L.off_sidx = o;   o = align_up(o + n * 4);
     L.off_skey = o;   o = align_up(o + n * 4);
     L.off_evoff = o;  o = align_up(o + static_cast<size_t>(n_events + 1) * 8);
@@ -142,11 +144,13 @@ struct Call {                 // everything that determines the enqueued work (a
     std::vector<int64_t> ev_off;
     bool timeline = false;
     bool dense = false;           // frnn_build_dense_ex: brute force instead of the grid
+    BinOrder order = {0, {0, 1, 2, 3, 4, 5, 6, 7}};
     bool operator==(const Call& o) const {
         return points == o.points && dim == o.dim && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
                out_dst == o.out_dst && out_d2 == o.out_d2 && capacity == o.capacity && out_count == o.out_count &&
                out_edge_offsets == o.out_edge_offsets && out_status == o.out_status && out_row_ptr == o.out_row_ptr &&
-               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline && dense == o.dense;
+               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline && dense == o.dense &&
+               order.on == o.order.on && memcmp(order.p, o.order.p, 8) == 0;
     }
 };
 
@@ -162,6 +166,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
     float4* spts_hi = c.dim > kDim ? reinterpret_cast<float4*>(ws + L.off_spts_hi) : nullptr;
+    uint32_t* scell = c.order.on ? reinterpret_cast<uint32_t*>(ws + L.off_scell) : nullptr;
     int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
     uint32_t* skey = reinterpret_cast<uint32_t*>(ws + L.off_skey);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
@@ -189,7 +194,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
         ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = 1; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
         ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
         ea.out_edge_offsets = nullptr; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
-        ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = nullptr; ea.dense = 1;
+        ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = nullptr; ea.dense = 1; ea.order = c.order;
         if (L.emit_tiles > kPrefixTilesMin) {
             unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
             tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
@@ -217,17 +222,18 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     }
     mark(0, st);
     const unsigned row_blocks = static_cast<unsigned>((n_total + 255) / 256);
-    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, stamps)));
+    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, c.order, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(1, st);
     cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor, stamps);
     ++t_launches; CK(cudaGetLastError());
     mark(2, st);
-    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, spts_hi, stamps)));
+    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, spts_hi, scell, c.order, stamps)));
     ++t_launches; CK(cudaGetLastError());
     mark(3, st);
 
     SearchArgs sa;
+    sa.scell = scell;
     sa.spts = spts; sa.spts_hi = spts_hi; sa.sidx = sidx; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
     sa.tile_deg = tile_deg; sa.n_tiles = static_cast<uint32_t>(L.emit_tiles); sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
     sa.inv_cell = inv_cell; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
@@ -242,7 +248,7 @@ int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
     ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
     ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
     ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
-    ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps; ea.dense = 0;
+    ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps; ea.dense = 0; ea.order = c.order;
     if (L.emit_tiles > kPrefixTilesMin) {                      // many tiles: their prefix in one small kernel (see tile_prefix_kernel)
         unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
         tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
@@ -273,7 +279,7 @@ int run_call(const Call& c, cudaStream_t st) {
         CK(cudaMemsetAsync(c.out_status, 0, 4, st)); ++t_launches;
         return FRNN_OK;
     }
-    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits}, c.dim);
+    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits}, c.dim, c.order.on != 0);
     bool graph_ok = g_use_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
     if (graph_ok) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
@@ -321,8 +327,9 @@ int prepare(Call& c, size_t workspace_bytes) {
     c.grid_dims = g.dims;
     c.grid_bits = g.bits;
     c.timeline = g_timeline;
+    c.order = g_order;
     if (n_total == 0) return FRNN_OK;
-    const Layout L = make_layout(n_total, c.n_events, g, c.dim);
+    const Layout L = make_layout(n_total, c.n_events, g, c.dim, c.order.on != 0);
     if (!c.workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
     if (reinterpret_cast<uintptr_t>(c.workspace) % kAlign) return FRNN_ERR_INVALID_ARG;
     return FRNN_OK;
@@ -371,7 +378,7 @@ const char* frnn_status_string(int status) {
 
 size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max) {
     if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDimMax || k_max < 1 || n_total > 0x7fffffffll) return 0;
-    return make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim).total;
+    return make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim, g_order.on != 0).total;
 }
 
 int frnn_set_grid(int grid_dims, int grid_bits) {
@@ -385,6 +392,81 @@ void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits
     const GridChoice g = choose_grid(n_total, n_events < 1 ? 1 : n_events);
     if (grid_dims) *grid_dims = g.dims;
     if (grid_bits) *grid_bits = g.bits;
+}
+
+int frnn_set_bin_order(const int* order, int count) {
+    if (count < 0 || count > 8 || (count > 0 && !order)) return FRNN_ERR_INVALID_ARG;
+    BinOrder o = {count > 0 ? 1 : 0, {0, 1, 2, 3, 4, 5, 6, 7}};
+    bool used[kDimMax] = {};
+    for (int k = 0; k < count; ++k) {
+        if (order[k] < 0 || order[k] >= kDimMax || used[order[k]]) return FRNN_ERR_INVALID_ARG;
+        used[order[k]] = true;
+        o.p[k] = static_cast<unsigned char>(order[k]);
+    }
+    int next = 0;
+    for (int k = count; k < 8; ++k) {                  // the rest: the unused coordinates in ascending order
+        while (used[next]) ++next;
+        used[next] = true;
+        o.p[k] = static_cast<unsigned char>(next);
+    }
+    g_order = o;
+    return FRNN_OK;
+}
+
+namespace {
+// Per coordinate: the probability that two random points of the sample fall within one cell of each other
+// (cells of side r, modulo 64) = sum_c p_c (p_{c-1} + p_c + p_{c+1}).  The smaller, the more that coordinate prunes.
+constexpr int kSuggestBins = 64;
+__global__ void __launch_bounds__(1024) suggest_kernel(const float* __restrict__ pts, int64_t n, int dim, float inv_cell,
+                                                       int64_t stride, float* __restrict__ out /* kDimMax */) {
+    __shared__ unsigned int s_h[kDimMax][kSuggestBins];
+    for (int k = threadIdx.x; k < kDimMax * kSuggestBins; k += blockDim.x) (&s_h[0][0])[k] = 0u;
+    __syncthreads();
+    unsigned int mine = 0;
+    for (int64_t i = static_cast<int64_t>(threadIdx.x) * stride; i < n; i += static_cast<int64_t>(blockDim.x) * stride) {
+        for (int d = 0; d < dim; ++d) atomicAdd(&s_h[d][cell_coord(pts[i * dim + d], inv_cell, kSuggestBins - 1)], 1u);
+        ++mine;
+    }
+    __shared__ unsigned int s_total;
+    if (threadIdx.x == 0) s_total = 0;
+    __syncthreads();
+    atomicAdd(&s_total, mine);
+    __syncthreads();
+    if (threadIdx.x < kDimMax) {
+        const int d = threadIdx.x;
+        double acc = 0.0;
+        const double tot = s_total ? static_cast<double>(s_total) : 1.0;
+        for (int c = 0; c < kSuggestBins; ++c) {
+            const double pc = s_h[d][c] / tot;
+            const double nb = (s_h[d][(c + kSuggestBins - 1) % kSuggestBins] + s_h[d][c] + s_h[d][(c + 1) % kSuggestBins]) / tot;
+            acc += pc * nb;
+        }
+        out[d] = d < dim ? static_cast<float>(acc) : 2.0f;          // absent coordinates prune nothing: last
+    }
+}
+}  // namespace
+
+int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int* order, float* score, void* cuda_stream) {
+    if (!points || !order || n < 1 || !(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
+    if (dim < 1 || dim > kDimMax) return FRNN_ERR_UNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    float* d_out = nullptr;
+    if (cudaMalloc(reinterpret_cast<void**>(&d_out), kDimMax * sizeof(float)) != cudaSuccess) return FRNN_ERR_CUDA;
+    const int64_t stride = n > 65536 ? n / 65536 : 1;              // a sample of at most ~65k points
+    const float inv_cell = 1.0f / fmaxf(r * kCellSlack, 1e-30f);
+    suggest_kernel<<<1, 1024, 0, st>>>(points, n, dim, inv_cell, stride, d_out);
+    float h[kDimMax];
+    const cudaError_t e = cudaMemcpyAsync(h, d_out, sizeof(h), cudaMemcpyDeviceToHost, st);
+    const cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaFree(d_out);
+    if (e != cudaSuccess || e2 != cudaSuccess) return FRNN_ERR_CUDA;
+    int idx[kDimMax];
+    for (int d = 0; d < kDimMax; ++d) idx[d] = d;
+    for (int a = 1; a < kDimMax; ++a)                               // stable insertion sort by score
+        for (int b = a; b > 0 && h[idx[b]] < h[idx[b - 1]]; --b) { const int t = idx[b]; idx[b] = idx[b - 1]; idx[b - 1] = t; }
+    for (int k = 0; k < 8; ++k) order[k] = idx[k];
+    if (score) for (int d = 0; d < kDimMax; ++d) score[d] = h[d];
+    return FRNN_OK;
 }
 
 int frnn_set_graph_mode(int enabled) {
@@ -636,7 +718,7 @@ int frnn_get_profile(float* phase_ms, int max_phases) {
 
 int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, int dim, double* begin_us, double* end_us, int max_phases) {
     if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1 || dim < 1 || dim > kDimMax) return FRNN_ERR_INVALID_ARG;
-    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim);
+    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim, g_order.on != 0);
     unsigned long long h[2 * kTimelinePhases];
     if (cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess)
         return FRNN_ERR_CUDA;

@@ -77,6 +77,38 @@ __device__ __forceinline__ uint32_t key_of_point(const float4& a, const float4& 
     return key;
 }
 
+// Caller-chosen coordinates (frnn_set_bin_order): p[0..G-1] are the binned coordinates, p[G..G+3]
+// the key coordinates.  ANY choice is exact (each binned or keyed coordinate is a necessary condition on its own,
+// DESIGN.md R8); the choice only decides how much the grid and the filter prune.  The coordinates are read from the
+// caller's row (n x dim, coordinates >= dim read as 0); the internal rows keep the original order, so d2 is untouched.
+struct BinOrder {
+    int on;                       // 0: the first G coordinates are binned, the next four keyed (the default fast path)
+    unsigned char p[8];
+};
+template <int G>
+__device__ __forceinline__ uint32_t cell_ordered(const float* __restrict__ row, int dim, uint32_t event, float inv_cell, int bits,
+                                                 const BinOrder& o) {
+    const uint32_t mask = (1u << bits) - 1u;
+    uint32_t lin = event;
+#pragma unroll
+    for (int d = 0; d < G; ++d) {
+        const int c = o.p[d];
+        lin = (lin << bits) | cell_coord(c < dim ? row[c] : 0.0f, inv_cell, mask);
+    }
+    return lin;
+}
+template <int G>
+__device__ __forceinline__ uint32_t key_ordered(const float* __restrict__ row, int dim, float inv_cell, const BinOrder& o) {
+    uint32_t key = 0;
+#pragma unroll
+    for (int f = 0; f < 4; ++f)
+        if (G + f < kDim) {
+            const int c = o.p[G + f];
+            key |= cell_coord(c < dim ? row[c] : 0.0f, inv_cell, 63u) << (8 * f);
+        }
+    return key;
+}
+
 // DESIGN.md R3: the pinned fp32 order.  Explicit rounding intrinsics: nvcc may not contract,
 // reassociate or reorder them.  Each lane runs the whole chain for one (query, candidate) pair.
 __device__ __forceinline__ float d2_pinned(const float4& qa, const float4& qb, const float4& ca, const float4& cb) {
@@ -187,14 +219,14 @@ __global__ void __launch_bounds__(256) bin_kernel(const float* __restrict__ pts,
                                                   float inv_cell, int bits,
                                                   uint32_t* __restrict__ cell_count,
                                                   uint32_t* __restrict__ pcell, uint32_t* __restrict__ prank,
-                                                  unsigned long long* stamps) {
+                                                  BinOrder order, unsigned long long* stamps) {
     stamp_begin(stamps, 0);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < n_total) {
         float4 a, b;
         load_point(pts, i, dim, a, b);
         const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
-        const uint32_t lin = cell_of_point<G>(a, b, ev, inv_cell, bits);
+        const uint32_t lin = order.on ? cell_ordered<G>(pts + i * dim, dim, ev, inv_cell, bits, order) : cell_of_point<G>(a, b, ev, inv_cell, bits);
         pcell[i] = lin;
         prank[i] = atomicAdd(&cell_count[padded(lin, bits)], 1u);
     }
@@ -212,16 +244,18 @@ __global__ void __launch_bounds__(256) scatter_kernel(const float* __restrict__ 
                                                       const uint32_t* __restrict__ prank,
                                                       float4* __restrict__ spts, int32_t* __restrict__ sidx,
                                                       uint32_t* __restrict__ skey, float4* __restrict__ spts_hi,
-                                                      unsigned long long* stamps) {
+                                                      uint32_t* __restrict__ scell, BinOrder order, unsigned long long* stamps) {
     stamp_begin(stamps, 2);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (i < n_total) {
-        const uint32_t s = cell_start[padded(pcell[i], bits)] + prank[i];
+        const uint32_t lin = pcell[i];
+        const uint32_t s = cell_start[padded(lin, bits)] + prank[i];
+        if (scell) scell[s] = lin;                                 // a bin order is set: the search cannot recompute the cell from the row
         float4 a, b;
         load_point(pts, i, dim, a, b);
         store_row(spts + 2 * static_cast<int64_t>(s), a, b);      // one 32-byte sector, one transaction
         sidx[s] = static_cast<int32_t>(i);
-        skey[s] = key_of_point<G>(a, b, inv_cell);
+        skey[s] = order.on ? key_ordered<G>(pts + i * dim, dim, inv_cell, order) : key_of_point<G>(a, b, inv_cell);
         if (spts_hi) {                                             // dim > 8: coordinates 8..15 travel in a second row
             float4 c, d;
             load_point_hi(pts, i, dim, c, d);
@@ -447,6 +481,7 @@ struct SearchArgs {
     uint32_t n_tiles;             // ceil(n_total / kEmitThreads)
     const int64_t* ev_off;        // device event offsets or NULL for one event
     unsigned long long* stamps;   // NULL unless the timeline is being recorded
+    const uint32_t* scell;        // slot -> linear cell id, stored by scatter_kernel only when a bin order is set, else NULL
     int64_t n_total;
     int n_events;
     float r2, inv_cell;
@@ -508,7 +543,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     // the slot's cell, recomputed from its coordinates (the event from the row index: blocks of the cell-ordered
     // copy land in arrival order, so slots are not ordered by event)
     const uint32_t ev = a.ev_off ? static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, my_row)) : 0u;
-    const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, bits);
+    const uint32_t cell = a.scell ? a.scell[s] : cell_of_point<G>(qa, qb, ev, a.inv_cell, bits);
     const uint32_t c_last = cell & mask;
     const uint32_t lo = c_last ? c_last - 1u : 0u, hi = c_last < mask ? c_last + 1u : mask;
     unsigned long long* const my_tile_deg = a.tile_deg + static_cast<size_t>(blockIdx.x & (kDegSlices - 1)) * a.n_tiles;
@@ -883,6 +918,7 @@ struct EmitArgs {
     int bits;
     uint32_t k_max;
     int dense;                    // 1: no grid exists (frnn_build_dense_ex): recomputed rows scan their whole event
+    BinOrder order;
 };
 
 template <int G, bool INTERIOR>
@@ -1097,7 +1133,8 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
             load_point(a.pts, row, a.dim, qa, qb);
             uint32_t ev = 0;
             if (a.ev_off) ev = static_cast<uint32_t>(event_of_row(a.ev_off, a.n_events, row));
-            const uint32_t cell = cell_of_point<G>(qa, qb, ev, a.inv_cell, a.bits);
+            const uint32_t cell = a.order.on ? cell_ordered<G>(a.pts + row * a.dim, a.dim, ev, a.inv_cell, a.bits, a.order)
+                                             : cell_of_point<G>(qa, qb, ev, a.inv_cell, a.bits);
             bool interior = true;
 #pragma unroll
             for (int d = 0; d < G; ++d) {

@@ -60,6 +60,9 @@ _SIGNATURES = {
                                              _c.c_void_p, _c.c_void_p]),
     "frnn_host_pipeline_wait": (_c.c_int, [_c.c_void_p]),
     "frnn_host_pipeline_destroy": (None, [_c.c_void_p]),
+    "frnn_set_bin_order": (_c.c_int, [_c.POINTER(_c.c_int), _c.c_int]),
+    "frnn_suggest_bin_order": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.POINTER(_c.c_int), _c.POINTER(_c.c_float),
+                                          _c.c_void_p]),
     "frnn_release_cached": (None, []),
 }
 EXPORTED_SYMBOLS = tuple(_SIGNATURES)
@@ -354,3 +357,21 @@ class HostPipeline:
             self.close()
         except Exception:
             pass
+
+
+def frnn_set_bin_order(order=None) -> None:
+    """Coordinates to bin (first) and to key (next four); None / empty restores the default."""
+    order = [int(v) for v in (order or [])]
+    arr = (_c.c_int * max(len(order), 1))(*order)
+    _check(lib().frnn_set_bin_order(arr if order else None, len(order)), "frnn_set_bin_order")
+
+
+def frnn_suggest_bin_order(points: torch.Tensor, r: float, stream: torch.cuda.Stream | None = None):
+    """Data-driven ranking of the coordinates of ``points`` (device, n x dim): returns (order[8], score[16])."""
+    _require_cuda(points)
+    n, dim = points.shape
+    order, score = (_c.c_int * 8)(), (_c.c_float * 16)()
+    stream = stream or torch.cuda.current_stream(points.device)
+    _check(lib().frnn_suggest_bin_order(_ptr(points), n, dim, float(r), order, score, _c.c_void_p(stream.cuda_stream)),
+           "frnn_suggest_bin_order")
+    return list(order), list(score)

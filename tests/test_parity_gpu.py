@@ -417,3 +417,61 @@ def test_clustered_event_in_higher_dimension(F, dim):
         assert exp.count > 20000
         got, _ = run_gpu(F, x, r, k, capacity=exp.count + 8)
         assert_same(got, exp, r, f"clustered dim={dim} K={k}")
+
+
+# ---------------------------------------------------------------- which coordinates are binned
+@pytest.mark.parametrize("order", [[7, 6, 5, 4, 3, 2, 1, 0], [4, 5, 6, 7], [3], [2, 9, 0, 15, 1], [1, 3, 5, 7, 0, 2, 4, 6]])
+def test_bin_order_never_changes_the_result(F, order):
+    cfg = events.CONFIGS[1]
+    x = events.make_event(cfg)[:8000]
+    exp = oracle.frnn(x, cfg.r, 6, oracle.CELLS)
+    try:
+        F.frnn_set_bin_order(order)
+        got, _ = run_gpu(F, x, cfg.r, 6)
+    finally:
+        F.frnn_set_bin_order(None)
+    assert_same(got, exp, cfg.r, f"bin order {order}")
+
+
+def test_suggested_bin_order_on_an_anisotropic_embedding(F):
+    """An embedding whose first four coordinates carry almost no spread: binning them prunes nothing.  The suggested
+    order must rank the four wide coordinates first, give the same result, and be much faster than the default."""
+    rng = np.random.default_rng(5)
+    n, tracks = 60000, 6000
+    centres = rng.uniform(-1, 1, (tracks, 8))
+    centres[:, :4] *= 0.02                                               # squeezed coordinates
+    x = centres[rng.integers(0, tracks, n)] + rng.normal(0, 0.02, (n, 8))
+    x = np.ascontiguousarray(x.astype(np.float32))
+    r, k = 0.08, 64
+    exp = oracle.frnn(x, r, k, oracle.BRUTE)
+    pts = torch.from_numpy(x).cuda()
+    order, score = F.frnn_suggest_bin_order(pts, r)
+    assert sorted(order[:4]) == [4, 5, 6, 7], (order, score)
+    assert all(score[d] > 0.9 for d in range(4)) and all(score[d] < 0.3 for d in range(4, 8)) and score[8] == 2.0
+
+    def timed():
+        ws = F.Workspace(n, 1, k, exp.count + 8)
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            for _ in range(3):
+                res = F.frnn_build_ex(pts, r, k, ws=ws, stream=st)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            for _ in range(10):
+                res = F.frnn_build_ex(pts, r, k, ws=ws, stream=st)
+            b.record(st)
+            st.synchronize()
+        res.check()
+        s, d, q = (t.cpu().numpy() for t in res.trimmed())
+        return a.elapsed_time(b) / 10, Got(s, d, q)
+
+    t_default, got_default = timed()
+    try:
+        F.frnn_set_bin_order(order)
+        t_suggested, got_suggested = timed()
+    finally:
+        F.frnn_set_bin_order(None)
+    assert_same(got_default, exp, r, "anisotropic, default order")
+    assert_same(got_suggested, exp, r, "anisotropic, suggested order")
+    print(f"[bin order] default {t_default:.3f} ms, suggested {order} {t_suggested:.3f} ms")
+    assert t_suggested < 0.5 * t_default
