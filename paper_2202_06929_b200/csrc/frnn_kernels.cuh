@@ -569,9 +569,10 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     // hits[row * kSlot + pos] = (other, d2) for pos < kSlot on both rows.  The counts keep running beyond kSlot,
     // which tells emit_kernel to resolve that row by recomputation; min(cnt, k_max) is the number of increments
     // that found a value < k_max, so the per-tile capped degree totals are accumulated by the same increments.
-    auto drain = [&]() {
+    auto drain = [&](bool stash = false) {
         const int qn = static_cast<int>((qaddr - q_base) / kQBytes);
         qaddr = q_base;
+        uint32_t hs = 0;                                                 // hits noted in the (by now free) leftover list
         for (int i = 0; i < qn; i += kWide) {
             float4 ca[kWide], cb[kWide];
             int32_t cj[kWide];
@@ -602,6 +603,12 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
                 nh += ok[v];
             }
             if (nh == 0) continue;
+            if (stash && hs + nh <= static_cast<uint32_t>(kLeft)) {      // final drain: only note the hits, commit them all at the end
+#pragma unroll
+                for (int v = 0; v < kWide; ++v)
+                    if (ok[v]) { s_left[hs][tid] = make_uint2(static_cast<uint32_t>(cj[v]), __float_as_uint(d2[v])); ++hs; }
+                continue;
+            }
             uint32_t pos = atomicAdd(&a.cnt[my_row], nh);
             uint32_t pq[kWide];
 #pragma unroll
@@ -617,6 +624,26 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
                     if (pq[v] < a.k_max) atomicAdd(&my_tile_deg[cj[v] / kEmitThreads], 1ull);
                     ++pos;
                 }
+        }
+        if (hs) {                                                        // the noted hits: ONE atomic on my row, the partners' in flight by four
+            uint32_t pos = atomicAdd(&a.cnt[my_row], hs);
+            for (uint32_t i = 0; i < hs; i += kWide) {
+                uint2 e[kWide];
+                uint32_t pq[kWide];
+#pragma unroll
+                for (int v = 0; v < kWide; ++v)
+                    if (i + v < hs) { e[v] = s_left[i + v][tid]; pq[v] = atomicAdd(&a.cnt[e[v].x], 1u); }
+#pragma unroll
+                for (int v = 0; v < kWide; ++v)
+                    if (i + v < hs) {
+                        const int32_t cjv = static_cast<int32_t>(e[v].x);
+                        if (pos < kSlot) a.hits[static_cast<int64_t>(my_row) * kSlot + pos] = make_int2(cjv, static_cast<int>(e[v].y));
+                        if (pq[v] < kSlot) a.hits[static_cast<int64_t>(cjv) * kSlot + pq[v]] = make_int2(my_row, static_cast<int>(e[v].y));
+                        own_deg += pos < a.k_max;
+                        if (pq[v] < a.k_max) atomicAdd(&my_tile_deg[cjv / kEmitThreads], 1ull);
+                        ++pos;
+                    }
+            }
         }
     };
     // a run of candidate slots [j0, j1), kBatch keys in flight
@@ -737,7 +764,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
                 scan_run(a.cell_start[r + wrap_cell], a.cell_start[r + wrap_cell + 1u]);
             }
     }
-    drain();
+    drain(true);
     // per-tile degree totals: emit_kernel turns them into its global offsets without any inter-block wait
     if (own_deg) atomicAdd(&my_tile_deg[my_row / kEmitThreads], static_cast<unsigned long long>(own_deg));
     stamp_end(a.stamps, 3);
