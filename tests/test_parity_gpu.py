@@ -475,3 +475,29 @@ def test_suggested_bin_order_on_an_anisotropic_embedding(F):
     assert_same(got_suggested, exp, r, "anisotropic, suggested order")
     print(f"[bin order] default {t_default:.3f} ms, suggested {order} {t_suggested:.3f} ms")
     assert t_suggested < 0.5 * t_default
+
+
+@pytest.mark.parametrize("dim,order", [(5, None), (12, None), (12, [9, 3, 11, 0, 5]), (8, [6, 2])])
+def test_batched_other_dims_and_bin_orders(F, dim, order):
+    """The batched entry point with dim != 8 and with a caller-chosen bin order (ragged events, an empty one)."""
+    rng = np.random.default_rng(100 + dim)
+    sizes = [1500, 0, 37, 2600, 1]
+    parts = []
+    for m in sizes:
+        c = rng.uniform(-1, 1, (max(m // 8, 1), dim))
+        parts.append((c[rng.integers(0, len(c), m)] + rng.normal(0, 0.03, (m, dim))).astype(np.float32))
+    x = np.ascontiguousarray(np.concatenate(parts))
+    offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    r = 0.03 * np.sqrt(2 * dim)
+    exp, eoffs = oracle.frnn_batched(x, offs, r, 5)
+    assert eoffs[-1] > 3000
+    try:
+        F.frnn_set_bin_order(order)
+        res = F.frnn_build_batched(torch.from_numpy(x).cuda(), offs, r, 5)
+        torch.cuda.synchronize()
+    finally:
+        F.frnn_set_bin_order(None)
+    res.check()
+    assert np.array_equal(res.count.cpu().numpy(), eoffs)
+    s, d, q = (t.cpu().numpy() for t in res.trimmed())
+    assert np.array_equal(s, exp.src) and np.array_equal(d, exp.dst) and np.array_equal(H.bits(q), H.bits(exp.d2))
