@@ -481,8 +481,8 @@ def main() -> None:
         dt_sync = D.reduce_max(time.perf_counter() - t, rank)
         e_total_sync = D.reduce_sum(e_edges, rank)
         # the host pipeline: the same copies per event, but H2D of event i+1, build of event i and D2H of event i-1
-        # overlap (3 slots); every event's edges land in one of 4 rotating sets of pinned host buffers
-        depth = 3
+        # overlap (4 slots); every event's edges land in one of 5 rotating sets of pinned host buffers
+        depth = 4
         pipe = F.HostPipeline(n, k_max, cap, depth=depth)
         hb = [(torch.empty(cap, dtype=torch.int32).pin_memory(), torch.empty(cap, dtype=torch.int32).pin_memory(),
                torch.empty(cap, dtype=torch.float32).pin_memory(), torch.zeros(1, dtype=torch.int64).pin_memory())
@@ -496,7 +496,7 @@ def main() -> None:
         for i in range(args.e2e_steps):
             slot = hb[i % len(hb)]
             if i >= len(hb):
-                p_edges += int(slot[3][0])        # the result of step i - 4: complete, since only 3 events are in flight
+                p_edges += int(slot[3][0])        # the result of step i - (depth + 1): complete, since only `depth` events are in flight
             pipe.submit(pin_in[i % n_pin], r, *slot)
         pipe.wait()
         dt = time.perf_counter() - t

@@ -172,24 +172,25 @@ int frnn_build_host(const float* points /* HOST */, int64_t n, int dim, float r,
 /*
  * Host pipeline: the end-to-end path for a STREAM of events in host memory.  Each submit enqueues, on the next of
  * `depth` internal slots (one CUDA stream, one workspace, one set of device buffers each): the H2D copy of the
- * points, frnn_build_ex, and one kernel that writes the (device-known) number of edges straight into the caller's
- * host buffers -- so the H2D copy of event i+1, the build of event i and the D2H copy of event i-1 overlap and
- * nothing synchronises in between.
- *   create : n_max = largest event, edge_capacity = room (in edges) of every output buffer passed later (used
- *            rounded down to a multiple of 4, >= 4), depth = events in flight (1..16; 3 is enough).
- *   submit : points HOST n x 8 fp32 (pinned recommended); out_src/out_dst/out_d2/out_count HOST and PAGE-LOCKED
- *            (cudaHostAlloc / cudaHostRegister; FRNN_ERR_INVALID_ARG otherwise), 16-byte aligned.  Returns
- *            immediately unless all slots are busy (then it waits for the oldest).  The outputs are valid after
- *            frnn_host_pipeline_wait (or after `depth` further submits).  *out_count = number of edges, or
- *            -(needed) - 1 when the result has more than edge_capacity edges (then only edge_capacity are written).
- *   wait   : blocks until every submitted event is complete.
+ * points, frnn_build_ex and the copy of the edge COUNT to the host.  As soon as the host sees (at a later submit or
+ * in wait) that a build has completed, it hands the copy of exactly that many edges to the copy engine.  So the H2D
+ * copy of event i+1, the build of event i and the D2H copy of event i-1 overlap; the only blocking point is the
+ * retirement of the oldest event in flight.
+ *   create : n_max = largest event, edge_capacity = room (in edges) of every output buffer passed later,
+ *            depth = events in flight (1..16; 3 or 4 is enough).
+ *   submit : points HOST n x 8 fp32; out_src/out_dst/out_d2/out_count HOST (page-locked memory makes the copies
+ *            asynchronous and is what bench.py uses; pageable memory works, slower).  Returns immediately unless the
+ *            slot it needs is still busy (then it retires that event first).  The outputs of an event are valid after
+ *            frnn_host_pipeline_wait, or after `depth` further submits.  *out_count = number of edges, or -(needed) - 1
+ *            when the result has more than edge_capacity edges (then only edge_capacity are written).
+ *   wait   : blocks until every submitted event is complete (oldest first).
  * Not thread safe per pipeline; distinct pipelines are independent.
  */
 typedef struct frnn_host_pipeline frnn_host_pipeline;
 int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth, frnn_host_pipeline** out);
 int frnn_host_pipeline_submit(frnn_host_pipeline* pipeline, const float* points /* HOST */, int64_t n, float r,
-                              int32_t* out_src /* HOST pinned */, int32_t* out_dst /* HOST pinned */,
-                              float* out_d2 /* HOST pinned */, int64_t* out_count /* HOST pinned */);
+                              int32_t* out_src /* HOST */, int32_t* out_dst /* HOST */,
+                              float* out_d2 /* HOST */, int64_t* out_count /* HOST */);
 int frnn_host_pipeline_wait(frnn_host_pipeline* pipeline);
 void frnn_host_pipeline_destroy(frnn_host_pipeline* pipeline);
 

@@ -576,17 +576,20 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     return FRNN_OK;
 }
 
-// ---- host pipeline: H2D of event i+1, build of event i and D2H of event i-1 overlap (one stream per slot)
+// ---- host pipeline: H2D of event i+1, build of event i and D2H of event i-1 overlap (one stream per slot); the edge
+// copies are DMA transfers of exactly `count` edges, started by the host as soon as it sees a build completed
 struct frnn_host_pipeline {
+    enum State { FREE, BUILDING, COPYING };
     struct Slot {
         cudaStream_t stream = nullptr;
-        cudaEvent_t done = nullptr;
+        cudaEvent_t built = nullptr, done = nullptr;
         void* ws = nullptr;
         float* pts = nullptr;
         int32_t* src = nullptr; int32_t* dst = nullptr; float* d2 = nullptr;
-        int64_t* count = nullptr; int32_t* status = nullptr;     // device
-        int64_t* host_count = nullptr;                            // the caller's (pinned) count word of the pending submit
-        bool busy = false;
+        int64_t* count = nullptr;                                 // device: count (8 bytes) followed by status (4 bytes)
+        int64_t* pinned = nullptr;                                // page-locked mirror of the two words above
+        int32_t* h_src = nullptr; int32_t* h_dst = nullptr; float* h_d2 = nullptr; int64_t* h_count = nullptr;   // the caller's
+        State state = FREE;
     };
     std::vector<Slot> slots;
     int64_t n_max = 0, cap = 0;
@@ -595,35 +598,6 @@ struct frnn_host_pipeline {
 };
 
 namespace {
-// count edges (known only on the device) go straight into the caller's pinned host buffers: one kernel, no
-// intermediate synchronisation; 16-byte vectors, a small grid (PCIe, not the SMs, is the limit)
-__global__ void __launch_bounds__(256) copy_out_kernel(const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-                                                       const float* __restrict__ d2, const int64_t* __restrict__ count,
-                                                       const int32_t* __restrict__ status, int64_t cap,
-                                                       int32_t* h_src, int32_t* h_dst, float* h_d2, int64_t* h_count) {
-    const int64_t c = *count;
-    const int64_t e = c < cap ? c : cap;
-    const int64_t n4 = (e + 3) / 4;                              // buffers hold a multiple of 4 entries (cap rounded up)
-    const int64_t stride = static_cast<int64_t>(gridDim.x) * blockDim.x;
-    for (int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += stride) {
-        reinterpret_cast<int4*>(h_src)[i] = reinterpret_cast<const int4*>(src)[i];
-        reinterpret_cast<int4*>(h_dst)[i] = reinterpret_cast<const int4*>(dst)[i];
-        reinterpret_cast<float4*>(h_d2)[i] = reinterpret_cast<const float4*>(d2)[i];
-    }
-    if (blockIdx.x == 0 && threadIdx.x == 0) *h_count = *status == 0 ? c : -c - 1;   // negative: capacity exceeded, -(needed) - 1
-}
-
-#ifndef FRNN_COPY_BLOCKS
-#define FRNN_COPY_BLOCKS 32
-#endif
-constexpr int kCopyBlocks = FRNN_COPY_BLOCKS;
-
-bool is_pinned_host(const void* p) {
-    cudaPointerAttributes a;
-    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
-    return a.type == cudaMemoryTypeHost;
-}
-
 void pipeline_free(frnn_host_pipeline* p) {
     for (auto& s : p->slots) {
         if (s.stream) cudaStreamSynchronize(s.stream);
@@ -631,33 +605,77 @@ void pipeline_free(frnn_host_pipeline* p) {
         if (s.pts) cudaFree(s.pts);
         if (s.src) cudaFree(s.src);
         if (s.count) cudaFree(s.count);
+        if (s.pinned) cudaFreeHost(s.pinned);
+        if (s.built) cudaEventDestroy(s.built);
         if (s.done) cudaEventDestroy(s.done);
         if (s.stream) cudaStreamDestroy(s.stream);
     }
     delete p;
 }
+
+// The build of this slot has completed: its edge count is on the host, so the copy of exactly that many edges can be
+// handed to the copy engine (it then runs beside the builds and the H2D copies of the other slots).
+int pipeline_start_copy(frnn_host_pipeline* p, frnn_host_pipeline::Slot& s) {
+    const int64_t c = s.pinned[0];
+    const int32_t status = *reinterpret_cast<const int32_t*>(s.pinned + 1);
+    *s.h_count = status == 0 ? c : -c - 1;                       // negative: capacity exceeded, -(needed) - 1
+    const size_t e = static_cast<size_t>(c < p->cap ? c : p->cap);
+    if (e) {
+        CK(cudaMemcpyAsync(s.h_src, s.src, e * 4, cudaMemcpyDeviceToHost, s.stream));
+        CK(cudaMemcpyAsync(s.h_dst, s.dst, e * 4, cudaMemcpyDeviceToHost, s.stream));
+        CK(cudaMemcpyAsync(s.h_d2, s.d2, e * 4, cudaMemcpyDeviceToHost, s.stream));
+    }
+    CK(cudaEventRecord(s.done, s.stream));
+    s.state = frnn_host_pipeline::COPYING;
+    return FRNN_OK;
+}
+
+int pipeline_retire(frnn_host_pipeline* p, frnn_host_pipeline::Slot& s) {
+    if (s.state == frnn_host_pipeline::BUILDING) {
+        CK(cudaEventSynchronize(s.built));
+        const int rc = pipeline_start_copy(p, s);
+        if (rc != FRNN_OK) return rc;
+    }
+    if (s.state == frnn_host_pipeline::COPYING) {
+        CK(cudaEventSynchronize(s.done));
+        s.state = frnn_host_pipeline::FREE;
+    }
+    return FRNN_OK;
+}
+
+// builds that have finished in the meantime get their edge copies started (never blocks)
+int pipeline_poll(frnn_host_pipeline* p) {
+    for (auto& s : p->slots)
+        if (s.state == frnn_host_pipeline::BUILDING && cudaEventQuery(s.built) == cudaSuccess) {
+            const int rc = pipeline_start_copy(p, s);
+            if (rc != FRNN_OK) return rc;
+        }
+    cudaGetLastError();                                          // cudaErrorNotReady of the queries is not an error
+    return FRNN_OK;
+}
 }  // namespace
 
 int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth, frnn_host_pipeline** out) {
-    if (!out || n_max < 1 || k_max < 1 || edge_capacity < 4 || depth < 1 || depth > 16) return FRNN_ERR_INVALID_ARG;
+    if (!out || n_max < 1 || k_max < 1 || edge_capacity < 1 || depth < 1 || depth > 16) return FRNN_ERR_INVALID_ARG;
     if (dim != kDim) return FRNN_ERR_UNSUPPORTED;
     frnn_host_pipeline* p = new (std::nothrow) frnn_host_pipeline;
     if (!p) return FRNN_ERR_CUDA;
     p->n_max = n_max; p->k_max = k_max;
-    p->cap = edge_capacity / 4 * 4;                             // whole 16-byte vectors, never beyond the caller's room
+    p->cap = edge_capacity;
     p->ws_bytes = frnn_workspace_bytes(n_max, 1, dim, k_max);
     p->slots.resize(static_cast<size_t>(depth));
     for (auto& s : p->slots) {
         bool ok = cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&s.built, cudaEventDisableTiming) == cudaSuccess &&
                   cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming) == cudaSuccess &&
                   cudaMalloc(&s.ws, p->ws_bytes) == cudaSuccess &&
                   cudaMalloc(reinterpret_cast<void**>(&s.pts), static_cast<size_t>(n_max) * 32) == cudaSuccess &&
                   cudaMalloc(reinterpret_cast<void**>(&s.src), static_cast<size_t>(p->cap) * 12) == cudaSuccess &&
-                  cudaMalloc(reinterpret_cast<void**>(&s.count), 64) == cudaSuccess;
+                  cudaMalloc(reinterpret_cast<void**>(&s.count), 64) == cudaSuccess &&
+                  cudaMallocHost(reinterpret_cast<void**>(&s.pinned), 64) == cudaSuccess;
         if (!ok) { cudaGetLastError(); pipeline_free(p); return FRNN_ERR_CUDA; }
         s.dst = s.src + p->cap;
         s.d2 = reinterpret_cast<float*>(s.dst + p->cap);
-        s.status = reinterpret_cast<int32_t*>(s.count + 1);
     }
     *out = p;
     return FRNN_OK;
@@ -666,27 +684,28 @@ int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_ca
 int frnn_host_pipeline_submit(frnn_host_pipeline* p, const float* points, int64_t n, float r,
                               int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t* out_count) {
     if (!p || !points || !out_src || !out_dst || !out_d2 || !out_count || n < 1 || n > p->n_max) return FRNN_ERR_INVALID_ARG;
-    if (!is_pinned_host(out_src) || !is_pinned_host(out_dst) || !is_pinned_host(out_d2) || !is_pinned_host(out_count))
-        return FRNN_ERR_INVALID_ARG;                             // the copy-out kernel writes them directly
-    if ((reinterpret_cast<uintptr_t>(out_src) | reinterpret_cast<uintptr_t>(out_dst) | reinterpret_cast<uintptr_t>(out_d2)) % 16) return FRNN_ERR_INVALID_ARG;
     auto& s = p->slots[static_cast<size_t>(p->next)];
-    if (s.busy) { CK(cudaEventSynchronize(s.done)); s.busy = false; }
-    CK(cudaMemcpyAsync(s.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, s.stream));
-    const int rc = frnn_build_ex(s.pts, n, kDim, r, p->k_max, s.src, s.dst, s.d2, p->cap, s.count, s.status, nullptr, s.ws, p->ws_bytes, s.stream);
+    int rc = pipeline_retire(p, s);                              // the oldest event in flight: wait for it if it is still there
     if (rc != FRNN_OK) return rc;
-    copy_out_kernel<<<kCopyBlocks, 256, 0, s.stream>>>(s.src, s.dst, s.d2, s.count, s.status, p->cap, out_src, out_dst, out_d2, out_count);
-    CK(cudaGetLastError());
-    CK(cudaEventRecord(s.done, s.stream));
-    s.busy = true;
+    if ((rc = pipeline_poll(p)) != FRNN_OK) return rc;
+    CK(cudaMemcpyAsync(s.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, s.stream));
+    int32_t* d_status = reinterpret_cast<int32_t*>(s.count + 1);
+    rc = frnn_build_ex(s.pts, n, kDim, r, p->k_max, s.src, s.dst, s.d2, p->cap, s.count, d_status, nullptr, s.ws, p->ws_bytes, s.stream);
+    if (rc != FRNN_OK) return rc;
+    CK(cudaMemcpyAsync(s.pinned, s.count, 12, cudaMemcpyDeviceToHost, s.stream));
+    CK(cudaEventRecord(s.built, s.stream));
+    s.h_src = out_src; s.h_dst = out_dst; s.h_d2 = out_d2; s.h_count = out_count;
+    s.state = frnn_host_pipeline::BUILDING;
     p->next = (p->next + 1) % static_cast<int>(p->slots.size());
     return FRNN_OK;
 }
 
 int frnn_host_pipeline_wait(frnn_host_pipeline* p) {
     if (!p) return FRNN_ERR_INVALID_ARG;
-    for (auto& s : p->slots)
-        if (s.busy) { CK(cudaEventSynchronize(s.done)); s.busy = false; }
-    return FRNN_OK;
+    const int n = static_cast<int>(p->slots.size());
+    int rc = pipeline_poll(p);
+    for (int k = 0; k < n && rc == FRNN_OK; ++k) rc = pipeline_retire(p, p->slots[static_cast<size_t>((p->next + k) % n)]);   // oldest first
+    return rc;
 }
 
 void frnn_host_pipeline_destroy(frnn_host_pipeline* p) {

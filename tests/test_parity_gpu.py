@@ -311,13 +311,18 @@ def test_host_pipeline_overlapped_events(F):
         e = int(c.item())
         assert e == exp.count
         assert_same(Got(s[:e].numpy(), d[:e].numpy(), q[:e].numpy()), exp, cfg.r, "host pipeline")
-    # capacity overflow is reported through the count word; pageable outputs are refused
+    # capacity overflow is reported through the count word; pageable outputs work too
     small = F.HostPipeline(cfg.n, cfg.k_max, 1000, depth=1)
     small.submit(pins[0], cfg.r, *outs[0])
     small.wait()
     assert int(outs[0][3].item()) == -oracle.frnn(xs[0], cfg.r, cfg.k_max).count - 1
-    with pytest.raises(F.FrnnError):
-        pipe.submit(pins[0], cfg.r, torch.empty(cap, dtype=torch.int32), outs[0][1], outs[0][2], outs[0][3])
+    pageable = (torch.empty(cap, dtype=torch.int32), torch.empty(cap, dtype=torch.int32), torch.empty(cap, dtype=torch.float32),
+                torch.zeros(1, dtype=torch.int64))
+    pipe.submit(torch.from_numpy(xs[1]), cfg.r, *pageable)
+    pipe.wait()
+    exp1 = oracle.frnn(xs[1], cfg.r, cfg.k_max)
+    e1 = int(pageable[3].item())
+    assert e1 == exp1.count and np.array_equal(pageable[0][:e1].numpy(), exp1.src) and np.array_equal(pageable[1][:e1].numpy(), exp1.dst)
     small.close()
     pipe.close()
 
