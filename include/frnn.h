@@ -34,7 +34,13 @@
  *     reported in *out_status (device int32): FRNN_OK, or FRNN_ERR_CAPACITY when the edge count
  *     exceeds edge_capacity; then *out_count holds the needed size and only edges at positions
  *     < edge_capacity are written.
- *   - Thread safety: calls using distinct workspaces may run concurrently on distinct streams.
+ *   - Thread safety: frnn_build_ex/_opt/_dense_ex/_batched(_opt) calls that use DISTINCT workspaces may run
+ *     concurrently from different host threads on different streams (tests/test_parity_gpu.py runs two threads
+ *     against the oracle).  Per-call choices travel in a frnn_options argument; the process-wide setters below
+ *     (frnn_set_grid, frnn_set_bin_order, frnn_set_graph_mode) only change the DEFAULTS used by calls without
+ *     options: every call snapshots them once under a lock, and a workspace must be sized
+ *     (frnn_workspace_bytes[_opt]) with the same defaults / options as the call that uses it.
+ *     frnn_set_profiling(1) / frnn_get_profile are bench instrumentation and not thread safe.
  *     No C++ exception crosses this boundary.
  *   - There is no CPU fallback: without a CUDA device every compute entry point fails with
  *     FRNN_ERR_CUDA.
@@ -64,6 +70,38 @@ int frnn_version(void);
 /* Static string for a frnn_status value (never NULL). */
 const char* frnn_status_string(int status);
 
+/* Text of the last CUDA failure behind a FRNN_ERR_CUDA returned on THIS host thread ("call: message (name)"; "" if
+ * none yet).  The library clears the runtime's non-sticky error state before returning FRNN_ERR_CUDA. */
+const char* frnn_last_error_string(void);
+
+/*
+ * Per-call options.  Fill with frnn_options_init, change what is needed, pass to the *_opt entry
+ * points; NULL there means "the process defaults".  PAPER.md:69 (section 3.4): the paper's grid bins "three
+ * dimensions" of the embedding and notes that the cost of the cells grows as O(3^k k n) with the number k of binned
+ * coordinates; which and how many coordinates are binned, and how many cells the toroidal grid has per coordinate,
+ * never change the RESULT (R8/R9), only the amount of pruning and the size of the cell table.
+ *   grid_dims   number of binned coordinates, 1..6; 0 = automatic (from the event size)
+ *   grid_bits   log2 of the toroidal grid extent per binned coordinate, 2..8; 0 = automatic (5).  With fewer cells
+ *               than the data's extent / r, far-apart cells alias onto one table entry: exact, more candidates.
+ *   order       order[0..order_count) = coordinates (0..15, distinct) binned first and keyed next, as in
+ *               frnn_set_bin_order; order_count = 0: the first grid_dims coordinates are binned, the next four keyed
+ *   launch_mode FRNN_LAUNCH_DEFAULT (process default, see frnn_set_graph_mode), FRNN_LAUNCH_GRAPH, FRNN_LAUNCH_PLAIN
+ *   timeline    != 0: the kernels leave %globaltimer stamps in the workspace (frnn_get_timeline)
+ * struct_bytes must be sizeof(frnn_options) of the caller's header (frnn_options_init sets it).
+ */
+enum { FRNN_LAUNCH_DEFAULT = 0, FRNN_LAUNCH_GRAPH = 1, FRNN_LAUNCH_PLAIN = 2 };
+typedef struct frnn_options {
+    uint32_t struct_bytes;
+    int32_t grid_dims;
+    int32_t grid_bits;
+    int32_t order_count;
+    int32_t order[8];
+    int32_t launch_mode;
+    int32_t timeline;
+    int32_t reserved[4];
+} frnn_options;
+void frnn_options_init(frnn_options* opt);
+
 /*
  * Bytes of scratch needed for a call over n_total rows in n_events events (n_events = 1 for
  * frnn_build_ex).  Depends on the grid chosen from (n_total / n_events); 0 on invalid arguments.
@@ -71,40 +109,77 @@ const char* frnn_status_string(int status);
  * permutation, per-row counts and the CSR row pointer.  256-byte aligned base required.
  */
 size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max);
+/* The same for calls made with `opt` (NULL: the process defaults, i.e. frnn_workspace_bytes). */
+size_t frnn_workspace_bytes_opt(const frnn_options* opt, int64_t n_total, int n_events, int dim, int k_max);
 
 /*
- * Grid override for sweeps (process-global, affects later calls and frnn_workspace_bytes):
- * grid_dims = number of leading coordinates that are binned (1..6), grid_bits = log2 of the
- * toroidal grid extent per binned coordinate (2..8).  0 restores the automatic choice.  The
- * result never depends on the grid (R8/R9).  Returns FRNN_OK or FRNN_ERR_INVALID_ARG.
+ * Default grid (process-wide DEFAULT for calls without options; affects frnn_workspace_bytes as well, so set it
+ * before sizing workspaces): grid_dims = number of leading coordinates that are binned (1..6), grid_bits = log2 of
+ * the toroidal grid extent per binned coordinate (2..8).  0 restores the automatic choice.  The result never
+ * depends on the grid (R8/R9).  Returns FRNN_OK or FRNN_ERR_INVALID_ARG.
  */
 int frnn_set_grid(int grid_dims, int grid_bits);
-/* The grid a call over (n_total, n_events) would use. */
-void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits);
+/* The grid a call without options over (n_total, n_events, dim) would use. */
+void frnn_get_grid(int64_t n_total, int n_events, int dim, int* grid_dims, int* grid_bits);
+
+/*
+ * S1 from the data (section 3.4: the O(3^k k n) trade-off behind the paper's
+ * "three dimensions").  Looks at a sample (<= 65,536 rows, evenly strided) of `points` (DEVICE, n x dim; the rows
+ * of n_events events of about n / n_events rows each): per coordinate the histogram of the cell coordinate (cells of
+ * side r (1 + 2^-7), modulo 256), its minimum and maximum.  From the histograms folded to 2^bits cells it gets, per
+ * coordinate and per bits, the probability s that two random points fall within one cell of each other on that
+ * torus; the expected candidates per query of a grid are n * product of s over its binned coordinates, the survivors
+ * of the key filter that times the product of s(64 cells) over the keyed ones.  It then picks the (grid_dims,
+ * grid_bits) -- and, only when that is predicted to gain more than 10 %, an order of the coordinates -- that minimise
+ * a cost model of the path (table entries to zero and scan; per query: neighbour rows, keys, survivors; constants in
+ * DESIGN.md section 7), over grids whose table stays within 32 cells per point of an event, and writes the choice
+ * into *opt (which must have been initialised; launch_mode and timeline are left alone).  *report (optional)
+ * receives what it saw and what it predicts.  The statistics of an embedding belong to the trained model more than
+ * to the event: choose once per model and radius, reuse the options -- the per-event path stays reduction-free.
+ * SYNCHRONOUS (one small kernel, a stream synchronise).  Never changes any result.
+ */
+typedef struct frnn_grid_report {
+    int32_t grid_dims, grid_bits, reordered;
+    int64_t sampled;                 /* rows looked at */
+    float predicted_candidates;      /* per query, both directions */
+    float predicted_survivors;       /* candidates that pass the key filter, per query */
+    float predicted_us;              /* the cost model's figure for one call */
+    float extent_cells[16];          /* (max - min) / cell side per coordinate */
+    float pair_probability[16];      /* s at the chosen grid_bits per coordinate */
+    float key_probability[16];       /* s at the key filter's 64 cells per coordinate */
+} frnn_grid_report;
+int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, float r, frnn_options* opt /* HOST, in/out */,
+                      frnn_grid_report* report /* HOST, optional */, void* cuda_stream);
 
 /*
  * Which coordinates the grid bins and which the key filter tests (PAPER.md:69 says only that the
  * paper's grid uses "three dimensions" of the embedding, not which).  order[0..count) lists coordinate indices in
  * [0, 16), distinct; a call whose grid bins g coordinates bins order[0..g) and keys the next four; entries not given
  * are filled with the unused coordinates in ascending order.  count == 0 (or order == NULL) restores the default (the
- * first g coordinates binned, the next four keyed -- the fast path).  Process-global.  The RESULT never depends on the
+ * first g coordinates binned, the next four keyed -- the fast path).  Process-wide DEFAULT for calls without options.  The RESULT never depends on the
  * order: every binned or keyed coordinate is a necessary condition by itself (R8); only the amount of pruning
  * does.  The statistics of an embedding belong to the trained model, not to the event: choose once, reuse.
  * frnn_suggest_bin_order ranks the coordinates of a sample of `points` (DEVICE, n x dim) by the probability that two
  * random points fall within one cell (side r) of each other along that coordinate -- the smaller, the more it prunes --
  * writes the best eight to order[0..8) (HOST) and, if score != NULL, the 16 probabilities to score (HOST; absent
- * coordinates: 2.0).  Synchronous (one small kernel, one device allocation, a stream synchronise).
+ * coordinates: 2.0).  Synchronous (one small kernel, a stream synchronise).
  */
 int frnn_set_bin_order(const int* order /* HOST */, int count);
 int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int* order /* HOST, 8 */,
                            float* score /* HOST, 16, optional */, void* cuda_stream);
 
 /*
- * Launch mode (process-global).  1 (default): a call on a non-default stream replays a cached CUDA
- * graph of its kernels (keyed by every argument; built on first use, at most 128 kept, least
- * recently used evicted) -- about 1 us per kernel boundary instead of about 3 us per stream launch.
- * 0: kernels are launched one by one.  Calls on the legacy default stream, calls made while the
- * caller is itself capturing the stream, and profiled calls always launch one by one.
+ * Launch mode (process-wide DEFAULT for calls without options).  1 (default): a call on a non-default stream runs
+ * as ONE launch of an instantiated CUDA graph that belongs to the call's workspace.  The graph depends only on the
+ * SHAPE of the call (which kernels run: grid_dims, dim <= 8 or > 8, single event or batch, bin order on/off, brute
+ * force or grid) -- never on n, the pointers, r, k_max or the capacity: those are written into the graph's nodes
+ * before the launch (only the nodes whose values changed since the workspace's previous call), so events of
+ * different sizes and rotating buffers replay the same graph (section 3: events differ in size).
+ * First use of a (workspace, shape) pair builds the graph (about 0.1 ms, bench.py prints it); at most 64 are kept,
+ * least recently used evicted; threads on distinct workspaces do not wait for each other.  About 1 us per kernel
+ * boundary instead of about 3 us per stream launch.
+ * 0: kernels are launched one by one.  Calls on the legacy default stream, calls made while the caller is itself
+ * capturing the stream, and event-profiled calls always launch one by one.
  */
 int frnn_set_graph_mode(int enabled);
 
@@ -113,7 +188,7 @@ int frnn_set_graph_mode(int enabled);
  * workspace, output capacity assumed n*k_max edges (caller guarantees that much room, or at
  * least as many edges as the result has -- nothing is written beyond n*k_max).  SYNCHRONOUS:
  * returns after completion.  out_count is a HOST pointer (here and only here).
- * Not thread safe (shared cached workspace).
+ * Calls are serialised by an internal lock (shared cached workspace).
  */
 int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
                int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t* out_count /* HOST */);
@@ -131,6 +206,11 @@ int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
                   int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                   int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
                   void* workspace, size_t workspace_bytes, void* cuda_stream);
+/* frnn_build_ex with per-call options (opt == NULL: the process defaults); workspace >= frnn_workspace_bytes_opt(opt, ...). */
+int frnn_build_opt(const frnn_options* opt, const float* points, int64_t n, int dim, float r, int k_max,
+                   int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                   int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
  * The brute-force variant.  PAPER.md:57 (section 3.1): the graph can be built by querying every
@@ -157,13 +237,18 @@ int frnn_build_batched(const float* points, const int64_t* event_offsets /* HOST
                        int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                        int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+int frnn_build_batched_opt(const frnn_options* opt, const float* points, const int64_t* event_offsets /* HOST */, int n_events,
+                           int dim, float r, int k_max,
+                           int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                           int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
- * Host-buffer convenience (the end-to-end call bench.py times as "e2e"): points and all outputs
- * are HOST pointers (pinned memory makes the copies asynchronous); device staging buffers are
+ * Host-buffer convenience: points and all outputs are HOST pointers (pinned memory makes the copies
+ * asynchronous; `points` needs only the 4-byte alignment of a float array); device staging buffers are
  * cached inside the library.  Copies the points in, runs frnn_build_ex, copies count + edges
  * out, synchronises.  Returns FRNN_ERR_CAPACITY if the result has more than edge_capacity edges
- * (*out_count = needed size, nothing else copied).  Not thread safe.
+ * (*out_count = needed size, nothing else copied).  Calls are serialised by an internal lock (one shared cache).
  */
 int frnn_build_host(const float* points /* HOST */, int64_t n, int dim, float r, int k_max,
                     int32_t* out_src /* HOST */, int32_t* out_dst /* HOST */, float* out_d2 /* HOST */,
@@ -184,10 +269,14 @@ int frnn_build_host(const float* points /* HOST */, int64_t n, int dim, float r,
  *            frnn_host_pipeline_wait, or after `depth` further submits.  *out_count = number of edges, or -(needed) - 1
  *            when the result has more than edge_capacity edges (then only edge_capacity are written).
  *   wait   : blocks until every submitted event is complete (oldest first).
+ * Events of any size 1..n_max may follow each other: every slot replays one graph whatever n is.
  * Not thread safe per pipeline; distinct pipelines are independent.
  */
 typedef struct frnn_host_pipeline frnn_host_pipeline;
 int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth, frnn_host_pipeline** out);
+/* The same with options fixed for the pipeline's lifetime (NULL: the process defaults at creation). */
+int frnn_host_pipeline_create_opt(const frnn_options* opt, int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth,
+                                  frnn_host_pipeline** out);
 int frnn_host_pipeline_submit(frnn_host_pipeline* pipeline, const float* points /* HOST */, int64_t n, float r,
                               int32_t* out_src /* HOST */, int32_t* out_dst /* HOST */,
                               float* out_d2 /* HOST */, int64_t* out_count /* HOST */);

@@ -1,11 +1,20 @@
-// frnn.cu -- host side of the C ABI declared in include/frnn.h (argument checks, workspace layout,
-// launch sequence, CUDA-graph cache).  No CPU fallback: every compute entry point needs a CUDA device.
+// frnn.cu -- host side of the C ABI declared in include/frnn.h (argument checks, workspace layout, launch plan,
+// per-workspace CUDA-graph executables).  No CPU fallback: every compute entry point needs a CUDA device.
+//
+// A call is turned into a PLAN: one optional memset + a list of (kernel function, grid, by-value argument struct).
+// The plan is either launched node by node on the caller's stream, or -- the default on a non-default stream --
+// written into the nodes of an instantiated CUDA graph that belongs to the call's WORKSPACE and to the plan's shape
+// (the list of kernel functions): cudaGraphExecKernelNodeSetParams / cudaGraphExecMemsetNodeSetParams per node whose
+// grid or arguments changed since the last call, then one cudaGraphLaunch.  Nothing of the executable depends on n,
+// the pointers, r, k_max or the capacity, so a stream of events of different sizes replays ONE graph
+// (section 3: the latency "depends almost linearly on the number of spacepoints" -- events differ in size).
 #include "frnn_kernels.cuh"
 
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
 
+#include <memory>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -19,39 +28,97 @@ using namespace frnn;
 constexpr float kCellSlack = 1.0078125f;   // 1 + 2^-7, see cell_coord()
 constexpr size_t kAlign = 256;
 constexpr int64_t kPrefixTilesMin = 1024;   // above this many emit tiles the tile offsets come from tile_prefix_kernel
-
-int g_force_dims = 0, g_force_bits = 0;
-int g_use_graph = 1;
-BinOrder g_order = {0, {0, 1, 2, 3, 4, 5, 6, 7}};   // frnn_set_bin_order
-bool g_timeline = false;                    // frnn_set_profiling(2): kernels leave %globaltimer stamps in the workspace
 constexpr int kTimelinePhases = 5;
 const char* const kTimelineNames[kTimelinePhases] = {"bin", "scan_cells", "scatter", "search", "emit"};
-thread_local int t_launches = 0;
-
-// Optional per-phase CUDA-event timing (frnn_set_profiling): one event after every phase.
 constexpr int kPhases = 6;
 const char* const kPhaseNames[kPhases] = {"memset", "bin", "scan_cells", "scatter", "search", "emit"};
+
+// ---- last CUDA error of this thread (frnn_last_error_string)
+thread_local char t_error[256] = "";
+int cuda_fail(cudaError_t e, const char* what) {
+    snprintf(t_error, sizeof(t_error), "%s: %s (%s)", what, cudaGetErrorString(e), cudaGetErrorName(e));
+    cudaGetLastError();                     // do not leave a non-sticky error behind for the caller's next check
+    return FRNN_ERR_CUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+
+// ---- per-call options; the process-wide defaults (frnn_set_grid / _bin_order / _graph_mode / _profiling(2)) are
+// snapshotted once per call under a mutex, so concurrent calls never see a half-written default
+struct Opts {
+    int grid_dims = 0, grid_bits = 0;       // 0 = automatic
+    BinOrder order = {0, {0, 1, 2, 3, 4, 5, 6, 7}};
+    bool use_graph = true;
+    bool timeline = false;
+};
+std::mutex g_defaults_mutex;
+Opts g_defaults;
+Opts default_opts() {
+    std::lock_guard<std::mutex> lock(g_defaults_mutex);
+    return g_defaults;
+}
+
+int make_order(const int* order, int count, BinOrder* out) {
+    if (count < 0 || count > 8 || (count > 0 && !order)) return FRNN_ERR_INVALID_ARG;
+    BinOrder o = {count > 0 ? 1 : 0, {0, 1, 2, 3, 4, 5, 6, 7}};
+    bool used[kDimMax] = {};
+    for (int k = 0; k < count; ++k) {
+        if (order[k] < 0 || order[k] >= kDimMax || used[order[k]]) return FRNN_ERR_INVALID_ARG;
+        used[order[k]] = true;
+        o.p[k] = static_cast<unsigned char>(order[k]);
+    }
+    int next = 0;
+    for (int k = count; k < 8; ++k) {                  // the rest: the unused coordinates in ascending order
+        while (used[next]) ++next;
+        used[next] = true;
+        o.p[k] = static_cast<unsigned char>(next);
+    }
+    bool identity = true;                              // the default order written out: take the fast path
+    for (int k = 0; k < 8; ++k) identity = identity && o.p[k] == k;
+    if (identity) o.on = 0;
+    *out = o;
+    return FRNN_OK;
+}
+
+int opts_from(const frnn_options* in, Opts* out) {
+    Opts o = default_opts();
+    if (in) {
+        if (in->struct_bytes < sizeof(frnn_options)) return FRNN_ERR_INVALID_ARG;
+        if (in->grid_dims < 0 || in->grid_dims > 6 || (in->grid_bits != 0 && (in->grid_bits < 2 || in->grid_bits > 8))) return FRNN_ERR_INVALID_ARG;
+        if (in->launch_mode < 0 || in->launch_mode > 2) return FRNN_ERR_INVALID_ARG;
+        o.grid_dims = in->grid_dims;
+        o.grid_bits = in->grid_bits;
+        const int rc = make_order(in->order, in->order_count, &o.order);
+        if (rc != FRNN_OK) return rc;
+        if (in->launch_mode == FRNN_LAUNCH_GRAPH) o.use_graph = true;
+        if (in->launch_mode == FRNN_LAUNCH_PLAIN) o.use_graph = false;
+        o.timeline = in->timeline != 0;
+    }
+    *out = o;
+    return FRNN_OK;
+}
+
+thread_local int t_launches = 0;
+
+// Optional per-phase CUDA-event timing (frnn_set_profiling(1)): one event after every phase.  Bench instrumentation,
+// process-global, not thread safe (documented).
 bool g_profiling = false;
 cudaEvent_t g_ev[kPhases + 1] = {};
 bool g_ev_valid = false;
-void mark(int phase_done, cudaStream_t st) {        // phase_done = -1: start of the call
-    if (g_profiling && g_ev_valid) cudaEventRecord(g_ev[phase_done + 1], st);
-}
 
 struct GridChoice { int dims, bits; };
 
-// Grid heuristic: cells per event = 2^(dims*bits).  Finer grids cut candidate rows per query
-// (3^dims cells of side ~r are visited) but cost table size and run bookkeeping; the switch points
-// come from the sweep recorded in DESIGN.md section 7.
-GridChoice choose_grid(int64_t n_total, int n_events, int dim = kDim) {
+// Grid: cells per event = 2^(dims*bits).  Finer grids cut candidate rows per query (3^dims cells of side ~r are
+// visited) but cost table size and run bookkeeping.  Without a caller's choice (frnn_options, from frnn_suggest_grid or
+// by hand) the grid follows the event size alone; the switch points come from the sweep in DESIGN.md section 7.
+GridChoice choose_grid(const Opts& o, int64_t n_total, int n_events, int dim) {
     const int64_t per_event = n_events > 0 ? (n_total + n_events - 1) / n_events : n_total;
     GridChoice g;
-    g.bits = g_force_bits ? g_force_bits : 5;
-    if (g_force_dims) g.dims = g_force_dims;
+    g.bits = o.grid_bits ? o.grid_bits : 5;
+    if (o.grid_dims) g.dims = o.grid_dims;
     else if (per_event < 16384) g.dims = 3;
     else if (per_event < 400000) g.dims = 4;
     else g.dims = 5;
-    if (!g_force_dims && g.dims > dim) g.dims = dim;          // binning a padded (all-zero) coordinate prunes nothing
+    if (!o.grid_dims && g.dims > dim) g.dims = dim;          // binning a padded (all-zero) coordinate prunes nothing
     int ev_bits = 0;
     while ((1ll << ev_bits) < n_events) ++ev_bits;
     while (g.dims * g.bits + ev_bits > 30 && g.dims > 1) --g.dims;     // padded table index stays below 2^31
@@ -70,7 +137,7 @@ struct Layout {
     size_t total;
 };
 
-Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim = kDim, bool ordered = false) {
+Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim, bool ordered) {
     Layout L;
     L.n_cells = static_cast<int64_t>(n_events) << (g.dims * g.bits);
     const int64_t row_len = (1ll << g.bits) + 1;
@@ -111,21 +178,21 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim = kDim, 
         default: { constexpr int GG = 6; EXPR; } break; \
     }
 
-#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return FRNN_ERR_CUDA; } while (0)
-
+// host_points: the pointer is only the source of a copy (frnn_build_host), so the 32-byte row alignment of the device
+// fast path does not apply to it
 int check_common(const float* points, int64_t n, int dim, float r, int k_max, const void* out_src, const void* out_dst,
-                 const void* out_d2, int64_t capacity) {
+                 const void* out_d2, int64_t capacity, bool host_points = false) {
     if (n < 0 || k_max < 1 || capacity < 0) return FRNN_ERR_INVALID_ARG;
     if (!(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
     if (n > 0 && !points) return FRNN_ERR_INVALID_ARG;
     if (dim < 1 || dim > kDimMax) return FRNN_ERR_UNSUPPORTED;
-    if (reinterpret_cast<uintptr_t>(points) % (dim == kDim ? 32 : 4)) return FRNN_ERR_INVALID_ARG;   // 8-float rows move as 256-bit transactions
+    if (reinterpret_cast<uintptr_t>(points) % ((dim == kDim && !host_points) ? 32 : 4)) return FRNN_ERR_INVALID_ARG;   // 8-float rows move as 256-bit transactions
     if (capacity > 0 && (!out_src || !out_dst || !out_d2)) return FRNN_ERR_INVALID_ARG;
     if (n > 0x7fffffffll) return FRNN_ERR_UNSUPPORTED;
     return FRNN_OK;
 }
 
-struct Call {                 // everything that determines the enqueued work (also the graph-cache key)
+struct Call {                 // everything that determines the enqueued work
     const float* points;
     int dim = kDim;
     int n_events;
@@ -141,133 +208,282 @@ struct Call {                 // everything that determines the enqueued work (a
     int64_t* out_row_ptr;
     void* workspace;
     int grid_dims, grid_bits;
-    std::vector<int64_t> ev_off;
-    bool timeline = false;
+    const int64_t* ev_off;        // HOST, n_events + 1
     bool dense = false;           // frnn_build_dense_ex: brute force instead of the grid
-    BinOrder order = {0, {0, 1, 2, 3, 4, 5, 6, 7}};
-    bool operator==(const Call& o) const {
-        return points == o.points && dim == o.dim && n_events == o.n_events && r == o.r && k_max == o.k_max && out_src == o.out_src &&
-               out_dst == o.out_dst && out_d2 == o.out_d2 && capacity == o.capacity && out_count == o.out_count &&
-               out_edge_offsets == o.out_edge_offsets && out_status == o.out_status && out_row_ptr == o.out_row_ptr &&
-               workspace == o.workspace && grid_dims == o.grid_dims && grid_bits == o.grid_bits && ev_off == o.ev_off && timeline == o.timeline && dense == o.dense &&
-               order.on == o.order.on && memcmp(order.p, o.order.p, 8) == 0;
-    }
+    Opts opts;
 };
 
-// The whole path, enqueued kernel by kernel on `st`.
-int enqueue(const Call& c, const Layout& L, cudaStream_t st) {
+// ------------------------------------------------------------------------------------------------
+// The plan of a call
+// ------------------------------------------------------------------------------------------------
+struct Node {
+    const void* func;
+    unsigned grid_x, grid_y, block;
+    int phase;                    // kPhaseNames index (per-phase event timing)
+    uint32_t arg_off, arg_bytes;  // the by-value argument struct inside Plan::args
+};
+struct Plan {
+    void* ms_dst = nullptr;
+    size_t ms_bytes = 0;
+    std::vector<Node> nodes;
+    std::vector<unsigned char> args;
+    void clear() { ms_dst = nullptr; ms_bytes = 0; nodes.clear(); args.clear(); }
+    template <class A>
+    void add(const void* func, unsigned grid_x, unsigned grid_y, unsigned block, int phase, const A& a) {
+        static_assert(sizeof(A) <= 4096, "kernel arguments are limited to 4 KB");
+        const size_t off = (args.size() + 15) & ~static_cast<size_t>(15);
+        args.resize(off + sizeof(A));
+        memcpy(args.data() + off, &a, sizeof(A));
+        nodes.push_back(Node{func, grid_x, grid_y, block, phase, static_cast<uint32_t>(off), static_cast<uint32_t>(sizeof(A))});
+    }
+};
+thread_local Plan t_plan;         // reused: a call allocates nothing once the vectors have grown
+
+template <class K> const void* fptr(K k) { return reinterpret_cast<const void*>(k); }
+
+// The whole path as a plan.
+void make_plan(const Call& c, const Layout& L, Plan& P) {
+    P.clear();
     const int64_t n_total = c.ev_off[c.n_events];
     char* ws = static_cast<char*>(c.workspace);
     uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
     unsigned long long* tile_deg = reinterpret_cast<unsigned long long*>(ws + L.off_tiles);
     unsigned int* cursor = reinterpret_cast<unsigned int*>(ws + L.off_counters);
-    unsigned long long* stamps = c.timeline ? reinterpret_cast<unsigned long long*>(ws + L.off_counters + 64) : nullptr;
+    unsigned long long* stamps = c.opts.timeline ? reinterpret_cast<unsigned long long*>(ws + L.off_counters + 64) : nullptr;
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
     float4* spts_hi = c.dim > kDim ? reinterpret_cast<float4*>(ws + L.off_spts_hi) : nullptr;
-    uint32_t* scell = c.order.on ? reinterpret_cast<uint32_t*>(ws + L.off_scell) : nullptr;
+    uint32_t* scell = c.opts.order.on ? reinterpret_cast<uint32_t*>(ws + L.off_scell) : nullptr;
     int32_t* sidx = reinterpret_cast<int32_t*>(ws + L.off_sidx);
     uint32_t* skey = reinterpret_cast<uint32_t*>(ws + L.off_skey);
     uint32_t* cnt = reinterpret_cast<uint32_t*>(ws + L.off_cnt);
     int64_t* ev_off = reinterpret_cast<int64_t*>(ws + L.off_evoff);
     int2* hits = reinterpret_cast<int2*>(ws + L.off_hits);
+    unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
     const float* pts = c.points;
     const int G = c.grid_dims, bits = c.grid_bits;
+    const BinOrder order = c.opts.order;
 
     const float r2 = c.r * c.r;                               // R2: fl32(r*r), once, on the host
     const float cell_side = fmaxf(c.r * kCellSlack, 1e-30f);
     const float inv_cell = 1.0f / cell_side;
+    const unsigned emit_tiles = static_cast<unsigned>(L.emit_tiles);
 
-    mark(-1, st);
+    EmitArgs ea;
+    ea.pts = pts; ea.dim = c.dim; ea.cnt = cnt; ea.hits = hits; ea.tile_deg = tile_deg; ea.tile_prefix = nullptr;
+    ea.n_total = n_total; ea.row_ptr = c.out_row_ptr; ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2;
+    ea.capacity = c.capacity; ea.out_count = c.out_count; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
+    ea.k_max = static_cast<uint32_t>(c.k_max); ea.n_tiles = emit_tiles; ea.order = order;
+
     if (c.dense) {                                             // brute force: no table, no sort (single event)
-        CK(cudaMemsetAsync(ws + L.off_tiles, 0, L.zero_bytes - L.off_tiles, st)); ++t_launches;
+        P.ms_dst = ws + L.off_tiles;
+        P.ms_bytes = L.zero_bytes - L.off_tiles;
         DenseArgs da;
-        da.pts = pts; da.dim = c.dim; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = static_cast<uint32_t>(L.emit_tiles);
+        da.pts = pts; da.dim = c.dim; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = emit_tiles;
         da.n = n_total; da.r2 = r2; da.k_max = static_cast<uint32_t>(c.k_max);
         const unsigned T = static_cast<unsigned>((n_total + kDenseTile - 1) / kDenseTile);
-        if (c.dim > kDim) dense_search_kernel<true><<<dim3(T, T), kDenseTile, 0, st>>>(da);
-        else              dense_search_kernel<false><<<dim3(T, T), kDenseTile, 0, st>>>(da);
-        ++t_launches; CK(cudaGetLastError());
-        EmitArgs ea;
-        ea.pts = pts; ea.dim = c.dim; ea.spts = nullptr; ea.spts_hi = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.cnt = cnt; ea.hits = hits; ea.ev_off = nullptr;
-        ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = 1; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
-        ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
-        ea.out_edge_offsets = nullptr; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
-        ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = nullptr; ea.dense = 1; ea.order = c.order;
+        P.add(c.dim > kDim ? fptr(dense_search_kernel<true>) : fptr(dense_search_kernel<false>), T, T, kDenseTile, 4, da);
+        ea.spts = nullptr; ea.spts_hi = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.ev_off = nullptr; ea.n_events = 1;
+        ea.out_edge_offsets = nullptr; ea.stamps = nullptr; ea.dense = 1;
         if (L.emit_tiles > kPrefixTilesMin) {
-            unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
-            tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
-            ++t_launches; CK(cudaGetLastError());
+            P.add(fptr(tile_prefix_kernel), 1, 1, kPrefixThreads, 5, PrefixArgs{tile_deg, emit_tiles, tprefix});
             ea.tile_prefix = tprefix;
         }
-        emit_kernel<1><<<static_cast<unsigned>(L.emit_tiles), kEmitThreads, 0, st>>>(ea);
-        ++t_launches; CK(cudaGetLastError());
-        return FRNN_OK;
+        P.add(fptr(emit_kernel<1>), emit_tiles, 1, kEmitThreads, 5, ea);
+        return;
     }
-    CK(cudaMemsetAsync(ws, 0, L.zero_bytes, st)); ++t_launches;
+    P.ms_dst = ws;
+    P.ms_bytes = L.zero_bytes;
     // Event offsets reach the device as kernel arguments (no pageable-memory copy, which would
     // synchronise the host with the stream); a single event needs none (base 0).
     if (c.n_events > 1) {
         for (int first = 0; first <= c.n_events; first += OffsetChunk::kN) {
             OffsetChunk ch;
+            ch.ev_off = ev_off;
             ch.first = first;
             ch.count = (c.n_events + 1 - first) < OffsetChunk::kN ? (c.n_events + 1 - first) : OffsetChunk::kN;
             for (int k = 0; k < ch.count; ++k) ch.v[k] = c.ev_off[first + k];
-            set_offsets_kernel<<<1, OffsetChunk::kN, 0, st>>>(ch, ev_off);
-            ++t_launches; CK(cudaGetLastError());
+            for (int k = ch.count; k < OffsetChunk::kN; ++k) ch.v[k] = 0;
+            P.add(fptr(set_offsets_kernel), 1, 1, OffsetChunk::kN, 0, ch);
         }
     } else {
         ev_off = nullptr;
     }
-    mark(0, st);
     const unsigned row_blocks = static_cast<unsigned>((n_total + 255) / 256);
-    FRNN_DISPATCH_G(G, (bin_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, c.order, stamps)));
-    ++t_launches; CK(cudaGetLastError());
-    mark(1, st);
-    cell_scan_kernel<<<static_cast<unsigned>(L.scan_blocks), kCellThreads, 0, st>>>(cells, L.n_entries, L.rows_per_block, bits, cursor, stamps);
-    ++t_launches; CK(cudaGetLastError());
-    mark(2, st);
-    FRNN_DISPATCH_G(G, (scatter_kernel<GG><<<row_blocks, 256, 0, st>>>(pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, spts_hi, scell, c.order, stamps)));
-    ++t_launches; CK(cudaGetLastError());
-    mark(3, st);
+    BinArgs ba{pts, c.dim, n_total, ev_off, c.n_events, inv_cell, bits, cells, pcell, prank, order, stamps};
+    FRNN_DISPATCH_G(G, (P.add(fptr(bin_kernel<GG>), row_blocks, 1, 256, 1, ba)));
+    P.add(fptr(cell_scan_kernel), static_cast<unsigned>(L.scan_blocks), 1, kCellThreads, 2,
+          ScanArgs{cells, L.n_entries, L.rows_per_block, bits, cursor, stamps});
+    ScatterArgs sc{pts, c.dim, n_total, bits, inv_cell, cells, pcell, prank, spts, sidx, skey, spts_hi, scell, order, stamps};
+    FRNN_DISPATCH_G(G, (P.add(fptr(scatter_kernel<GG>), row_blocks, 1, 256, 3, sc)));
 
     SearchArgs sa;
     sa.scell = scell;
     sa.spts = spts; sa.spts_hi = spts_hi; sa.sidx = sidx; sa.skey = skey; sa.cell_start = cells; sa.cnt = cnt; sa.hits = hits;
-    sa.tile_deg = tile_deg; sa.n_tiles = static_cast<uint32_t>(L.emit_tiles); sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
+    sa.tile_deg = tile_deg; sa.n_tiles = emit_tiles; sa.ev_off = ev_off; sa.stamps = stamps; sa.n_total = n_total; sa.n_events = c.n_events; sa.r2 = r2;
     sa.inv_cell = inv_cell; sa.bits = bits; sa.k_max = static_cast<uint32_t>(c.k_max);
     const unsigned search_blocks = static_cast<unsigned>((n_total + kSearchThreads - 1) / kSearchThreads);
-    if (spts_hi) { FRNN_DISPATCH_G(G, (search_kernel<GG, true><<<search_blocks, kSearchThreads, 0, st>>>(sa))); }
-    else         { FRNN_DISPATCH_G(G, (search_kernel<GG, false><<<search_blocks, kSearchThreads, 0, st>>>(sa))); }
-    ++t_launches; CK(cudaGetLastError());
-    mark(4, st);
+    if (spts_hi) { FRNN_DISPATCH_G(G, (P.add(fptr(search_kernel<GG, true>), search_blocks, 1, kSearchThreads, 4, sa))); }
+    else         { FRNN_DISPATCH_G(G, (P.add(fptr(search_kernel<GG, false>), search_blocks, 1, kSearchThreads, 4, sa))); }
 
-    EmitArgs ea;
-    ea.pts = pts; ea.dim = c.dim; ea.spts = spts; ea.spts_hi = spts_hi; ea.sidx = sidx; ea.cell_start = cells; ea.cnt = cnt; ea.hits = hits; ea.ev_off = ev_off;
-    ea.tile_deg = tile_deg; ea.tile_prefix = nullptr; ea.n_events = c.n_events; ea.n_total = n_total; ea.row_ptr = c.out_row_ptr;
-    ea.out_src = c.out_src; ea.out_dst = c.out_dst; ea.out_d2 = c.out_d2; ea.capacity = c.capacity; ea.out_count = c.out_count;
-    ea.out_edge_offsets = c.out_edge_offsets; ea.out_status = c.out_status; ea.r2 = r2; ea.inv_cell = inv_cell; ea.bits = bits;
-    ea.k_max = static_cast<uint32_t>(c.k_max); ea.stamps = stamps; ea.dense = 0; ea.order = c.order;
+    ea.spts = spts; ea.spts_hi = spts_hi; ea.sidx = sidx; ea.cell_start = cells; ea.ev_off = ev_off; ea.n_events = c.n_events;
+    ea.out_edge_offsets = c.out_edge_offsets; ea.stamps = stamps; ea.dense = 0;
     if (L.emit_tiles > kPrefixTilesMin) {                      // many tiles: their prefix in one small kernel (see tile_prefix_kernel)
-        unsigned long long* tprefix = reinterpret_cast<unsigned long long*>(ws + L.off_tprefix);
-        tile_prefix_kernel<<<1, kPrefixThreads, 0, st>>>(tile_deg, static_cast<uint32_t>(L.emit_tiles), tprefix);
-        ++t_launches; CK(cudaGetLastError());
+        P.add(fptr(tile_prefix_kernel), 1, 1, kPrefixThreads, 5, PrefixArgs{tile_deg, emit_tiles, tprefix});
         ea.tile_prefix = tprefix;
     }
-    FRNN_DISPATCH_G(G, (emit_kernel<GG><<<static_cast<unsigned>(L.emit_tiles), kEmitThreads, 0, st>>>(ea)));
-    ++t_launches; CK(cudaGetLastError());
-    mark(5, st);
+    FRNN_DISPATCH_G(G, (P.add(fptr(emit_kernel<GG>), emit_tiles, 1, kEmitThreads, 5, ea)));
+}
+
+// ---- the plan launched node by node (legacy default stream, a capturing caller, graph mode off, per-phase events)
+int launch_plain(const Plan& P, cudaStream_t st) {
+    const bool prof = g_profiling && g_ev_valid;
+    int cur = 0;                                              // events recorded so far = cur + 1
+    if (prof) cudaEventRecord(g_ev[0], st);
+    CK(cudaMemsetAsync(P.ms_dst, 0, P.ms_bytes, st));
+    ++t_launches;
+    for (const Node& nd : P.nodes) {
+        if (prof) for (; cur < nd.phase; ++cur) cudaEventRecord(g_ev[cur + 1], st);
+        void* argp = const_cast<unsigned char*>(P.args.data() + nd.arg_off);
+        CK(cudaLaunchKernel(nd.func, dim3(nd.grid_x, nd.grid_y), dim3(nd.block), &argp, 0, st));
+        ++t_launches;
+    }
+    if (prof) for (; cur < kPhases; ++cur) cudaEventRecord(g_ev[cur + 1], st);
     return FRNN_OK;
 }
 
-// ---- CUDA-graph cache: the same call (same pointers, sizes, parameters) replays one instantiated
-// graph, which costs ~1 us per kernel boundary instead of ~3 us per stream launch (profiles/).
-struct CachedGraph { Call key; cudaGraphExec_t exec; int launches; uint64_t stamp; };
-std::vector<CachedGraph> g_graphs;
-std::mutex g_graph_mutex;
+// ------------------------------------------------------------------------------------------------
+// Per-workspace graph executables.  An entry belongs to (workspace pointer, shape = list of kernel functions); a
+// workspace sees few shapes (the grid changes with the event-size class, dense vs grid, batched chunk count), so a
+// handful of entries per workspace and kMaxExecs in total (least recently used evicted) are plenty.  The global mutex
+// covers only the lookup; update + launch run under the entry's own mutex, so threads that use distinct workspaces
+// (the contract of include/frnn.h) never wait for each other.
+// ------------------------------------------------------------------------------------------------
+struct ExecEntry {
+    void* workspace = nullptr;
+    std::vector<const void*> funcs;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraphNode_t ms_node = nullptr;
+    std::vector<cudaGraphNode_t> knodes;
+    Plan held;                    // the parameters the executable currently holds
+    uint64_t stamp = 0;
+    std::mutex mu;
+    ~ExecEntry() { if (exec) cudaGraphExecDestroy(exec); }
+};
+std::vector<std::shared_ptr<ExecEntry>> g_execs;
+std::mutex g_exec_mutex;
 uint64_t g_stamp = 0;
-constexpr size_t kMaxGraphs = 128;
+constexpr size_t kMaxExecs = 64;
+
+bool same_shape(const ExecEntry& e, const Plan& P) {
+    if (e.funcs.size() != P.nodes.size()) return false;
+    for (size_t k = 0; k < P.nodes.size(); ++k)
+        if (e.funcs[k] != P.nodes[k].func) return false;
+    return true;
+}
+
+cudaKernelNodeParams node_params(const Node& nd, void** argp) {
+    cudaKernelNodeParams kp = {};
+    kp.func = const_cast<void*>(nd.func);
+    kp.gridDim = dim3(nd.grid_x, nd.grid_y);
+    kp.blockDim = dim3(nd.block);
+    kp.sharedMemBytes = 0;
+    kp.kernelParams = argp;
+    kp.extra = nullptr;
+    return kp;
+}
+cudaMemsetParams memset_params(const Plan& P) {
+    cudaMemsetParams mp = {};
+    mp.dst = P.ms_dst;
+    mp.pitch = 0;
+    mp.value = 0;
+    mp.elementSize = 1;
+    mp.width = P.ms_bytes;
+    mp.height = 1;
+    return mp;
+}
+
+// build the executable of entry e from plan P (explicit nodes, a linear chain)
+int build_exec(ExecEntry& e, const Plan& P) {
+    if (e.exec) { cudaGraphExecDestroy(e.exec); e.exec = nullptr; }
+    e.knodes.clear();
+    cudaGraph_t graph = nullptr;
+    CK(cudaGraphCreate(&graph, 0));
+    cudaError_t err;
+    const cudaMemsetParams mp = memset_params(P);
+    err = cudaGraphAddMemsetNode(&e.ms_node, graph, nullptr, 0, &mp);
+    cudaGraphNode_t prev = e.ms_node;
+    for (size_t k = 0; err == cudaSuccess && k < P.nodes.size(); ++k) {
+        void* argp = const_cast<unsigned char*>(P.args.data() + P.nodes[k].arg_off);
+        const cudaKernelNodeParams kp = node_params(P.nodes[k], &argp);
+        cudaGraphNode_t node = nullptr;
+        err = cudaGraphAddKernelNode(&node, graph, &prev, 1, &kp);
+        e.knodes.push_back(node);
+        prev = node;
+    }
+    if (err == cudaSuccess) err = cudaGraphInstantiate(&e.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (err != cudaSuccess) { e.exec = nullptr; return cuda_fail(err, "building the CUDA graph"); }
+    e.held = P;                                                // (e.funcs, the identity of the entry, was set at creation)
+    return FRNN_OK;
+}
+
+// write what changed since the last launch into the executable's nodes
+int update_exec(ExecEntry& e, const Plan& P) {
+    if (e.held.ms_dst != P.ms_dst || e.held.ms_bytes != P.ms_bytes) {
+        const cudaMemsetParams mp = memset_params(P);
+        const cudaError_t err = cudaGraphExecMemsetNodeSetParams(e.exec, e.ms_node, &mp);
+        if (err != cudaSuccess) return cuda_fail(err, "cudaGraphExecMemsetNodeSetParams");
+        e.held.ms_dst = P.ms_dst;
+        e.held.ms_bytes = P.ms_bytes;
+    }
+    if (e.held.args.size() != P.args.size()) e.held.args.assign(P.args.size(), 0);     // (same shape: same sizes, in fact)
+    for (size_t k = 0; k < P.nodes.size(); ++k) {
+        const Node& nd = P.nodes[k];
+        Node& old = e.held.nodes[k];
+        const unsigned char* src = P.args.data() + nd.arg_off;
+        unsigned char* dst = e.held.args.data() + nd.arg_off;
+        if (old.grid_x == nd.grid_x && old.grid_y == nd.grid_y && old.block == nd.block && memcmp(src, dst, nd.arg_bytes) == 0) continue;
+        void* argp = const_cast<unsigned char*>(src);
+        const cudaKernelNodeParams kp = node_params(nd, &argp);
+        const cudaError_t err = cudaGraphExecKernelNodeSetParams(e.exec, e.knodes[k], &kp);
+        if (err != cudaSuccess) return cuda_fail(err, "cudaGraphExecKernelNodeSetParams");
+        memcpy(dst, src, nd.arg_bytes);
+        old = nd;
+    }
+    return FRNN_OK;
+}
+
+int launch_graph(const Plan& P, void* workspace, cudaStream_t st) {
+    std::shared_ptr<ExecEntry> e;
+    {
+        std::lock_guard<std::mutex> lock(g_exec_mutex);
+        for (auto& x : g_execs)
+            if (x->workspace == workspace && same_shape(*x, P)) { e = x; break; }
+        if (!e) {
+            if (g_execs.size() >= kMaxExecs) {                 // evict the least recently used
+                size_t victim = 0;
+                for (size_t k = 1; k < g_execs.size(); ++k)
+                    if (g_execs[k]->stamp < g_execs[victim]->stamp) victim = k;
+                g_execs.erase(g_execs.begin() + victim);       // destroyed when its last user lets go
+            }
+            e = std::make_shared<ExecEntry>();
+            e->workspace = workspace;
+            for (const Node& nd : P.nodes) e->funcs.push_back(nd.func);
+            g_execs.push_back(e);
+        }
+        e->stamp = ++g_stamp;
+    }
+    std::lock_guard<std::mutex> lock(e->mu);
+    int rc = FRNN_OK;
+    if (!e->exec) rc = build_exec(*e, P);
+    else if ((rc = update_exec(*e, P)) != FRNN_OK) rc = build_exec(*e, P);     // an update the driver refuses: start over
+    if (rc != FRNN_OK) return rc;
+    CK(cudaGraphLaunch(e->exec, st));
+    t_launches = static_cast<int>(P.nodes.size()) + 1;
+    return FRNN_OK;
+}
 
 int run_call(const Call& c, cudaStream_t st) {
     t_launches = 0;
@@ -279,63 +495,69 @@ int run_call(const Call& c, cudaStream_t st) {
         CK(cudaMemsetAsync(c.out_status, 0, 4, st)); ++t_launches;
         return FRNN_OK;
     }
-    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits}, c.dim, c.order.on != 0);
-    bool graph_ok = g_use_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
+    const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits}, c.dim, c.opts.order.on != 0);
+    Plan& P = t_plan;
+    make_plan(c, L, P);
+    bool graph_ok = c.opts.use_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
     if (graph_ok) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) graph_ok = false;   // caller is capturing: just enqueue
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); graph_ok = false; }   // caller is capturing: just enqueue
     }
-    if (!graph_ok) return enqueue(c, L, st);
-
-    std::lock_guard<std::mutex> lock(g_graph_mutex);
-    for (auto& g : g_graphs) {
-        if (g.key == c) {
-            g.stamp = ++g_stamp;
-            t_launches = g.launches;
-            CK(cudaGraphLaunch(g.exec, st));
-            return FRNN_OK;
-        }
-    }
-    cudaGraph_t graph = nullptr;
-    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return enqueue(c, L, st); }
-    const int rc = enqueue(c, L, st);
-    const cudaError_t ce = cudaStreamEndCapture(st, &graph);
-    if (rc != FRNN_OK || ce != cudaSuccess || !graph) {
-        if (graph) cudaGraphDestroy(graph);
-        cudaGetLastError();
-        return rc != FRNN_OK ? rc : FRNN_ERR_CUDA;
-    }
-    cudaGraphExec_t exec = nullptr;
-    const cudaError_t ie = cudaGraphInstantiate(&exec, graph, 0);
-    cudaGraphDestroy(graph);
-    if (ie != cudaSuccess) { cudaGetLastError(); return FRNN_ERR_CUDA; }
-    if (g_graphs.size() >= kMaxGraphs) {      // evict the least recently used
-        size_t victim = 0;
-        for (size_t k = 1; k < g_graphs.size(); ++k)
-            if (g_graphs[k].stamp < g_graphs[victim].stamp) victim = k;
-        cudaGraphExecDestroy(g_graphs[victim].exec);
-        g_graphs.erase(g_graphs.begin() + victim);
-    }
-    g_graphs.push_back(CachedGraph{c, exec, t_launches, ++g_stamp});
-    CK(cudaGraphLaunch(exec, st));
-    return FRNN_OK;
+    if (!graph_ok) return launch_plain(P, st);
+    return launch_graph(P, c.workspace, st);
 }
 
 int prepare(Call& c, size_t workspace_bytes) {
     const int64_t n_total = c.ev_off[c.n_events];
-    const GridChoice g = choose_grid(n_total, c.n_events, c.dim);
+    const GridChoice g = choose_grid(c.opts, n_total, c.n_events, c.dim);
     c.grid_dims = g.dims;
     c.grid_bits = g.bits;
-    c.timeline = g_timeline;
-    c.order = g_order;
     if (n_total == 0) return FRNN_OK;
-    const Layout L = make_layout(n_total, c.n_events, g, c.dim, c.order.on != 0);
+    const Layout L = make_layout(n_total, c.n_events, g, c.dim, c.opts.order.on != 0);
     if (!c.workspace || workspace_bytes < L.total) return FRNN_ERR_WORKSPACE;
     if (reinterpret_cast<uintptr_t>(c.workspace) % kAlign) return FRNN_ERR_INVALID_ARG;
     return FRNN_OK;
 }
 
-// cached device buffers for the synchronous convenience entry points
+int build_single(const Opts& o, bool dense, const float* points, int64_t n, int dim, float r, int k_max,
+                 int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                 int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    if (rc != FRNN_OK) return rc;
+    if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
+    if (dense && n > 65535ll * kDenseTile) return FRNN_ERR_UNSUPPORTED;       // grid.y limit (8.3 M rows)
+    const int64_t ev_off[2] = {0, n};
+    Call c{points, dim, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, ev_off};
+    c.dense = dense;
+    c.opts = o;
+    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
+    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int build_batched(const Opts& o, const float* points, const int64_t* event_offsets, int n_events, int dim, float r, int k_max,
+                  int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                  int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
+                  void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (n_events < 1 || !event_offsets || event_offsets[0] != 0) return FRNN_ERR_INVALID_ARG;
+    for (int e = 0; e < n_events; ++e)
+        if (event_offsets[e + 1] < event_offsets[e]) return FRNN_ERR_INVALID_ARG;
+    int rc = check_common(points, event_offsets[n_events], dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    if (rc != FRNN_OK) return rc;
+    if (!out_edge_offsets || !out_status) return FRNN_ERR_INVALID_ARG;
+    Call c{points, dim, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets, out_status, out_row_ptr,
+           workspace, 0, 0, event_offsets};
+    c.opts = o;
+    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
+    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
+}
+
+size_t workspace_bytes_for(const Opts& o, int64_t n_total, int n_events, int dim, int k_max) {
+    if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDimMax || k_max < 1 || n_total > 0x7fffffffll) return 0;
+    return make_layout(n_total, n_events, choose_grid(o, n_total, n_events, dim), dim, o.order.on != 0).total;
+}
+
+// cached device buffers for the synchronous convenience entry points (one user at a time: g_cache_mutex)
 struct Cache {
     void* ws = nullptr; size_t ws_bytes = 0;
     void* misc = nullptr;                       // count (8) + status (4)
@@ -343,26 +565,151 @@ struct Cache {
     void* edges = nullptr; size_t edge_cap = 0; // src | dst | d2, edge_cap each
     cudaStream_t stream = nullptr;              // non-default stream so the graph path applies
 } g_cache;
+std::mutex g_cache_mutex;
 
 int ensure(void** p, size_t* have, size_t need) {
     if (*have >= need && *p) return FRNN_OK;
     if (*p) cudaFree(*p);
     *p = nullptr; *have = 0;
-    if (cudaMalloc(p, need) != cudaSuccess) return FRNN_ERR_CUDA;
+    CK(cudaMalloc(p, need));
     *have = need;
     return FRNN_OK;
 }
 
 int ensure_stream() {
-    if (!g_cache.stream && cudaStreamCreateWithFlags(&g_cache.stream, cudaStreamNonBlocking) != cudaSuccess) return FRNN_ERR_CUDA;
+    if (!g_cache.stream) CK(cudaStreamCreateWithFlags(&g_cache.stream, cudaStreamNonBlocking));
     return FRNN_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S1 from the data: per coordinate, the histogram of the cell coordinate (cells of side
+// r (1 + 2^-7), modulo 256) over a sample of the points, and the coordinate's minimum and maximum.  Folded to
+// 2^bits cells on the host, a histogram p gives  s(bits) = sum_c p_c (p_(c-1) + p_c + p_(c+1)),  the probability
+// that two random points fall within one cell of each other along that coordinate on a torus of 2^bits cells: the
+// factor by which binning (or keying) that coordinate cuts the candidates.  PAPER.md:69 (section 3.4): the cost of
+// the cells grows as O(3^k k n) in the number k of binned coordinates, which is why the paper stops at three; the
+// choice below weighs exactly that against the candidates saved.
+// ------------------------------------------------------------------------------------------------
+constexpr int kSugBins = 256;
+struct SuggestOut {
+    unsigned int hist[kDimMax][kSugBins];
+    float lo[kDimMax], hi[kDimMax];
+    unsigned int sampled;
+};
+struct SuggestArgs {
+    const float* pts;
+    int64_t n;
+    int dim;
+    float inv_cell;
+    int64_t stride;
+    SuggestOut* out;
+};
+__global__ void __launch_bounds__(1024) suggest_kernel(SuggestArgs k) {
+    __shared__ unsigned int s_h[kDimMax][kSugBins];
+    __shared__ float s_lo[kDimMax][32], s_hi[kDimMax][32];
+    for (int t = threadIdx.x; t < kDimMax * kSugBins; t += blockDim.x) (&s_h[0][0])[t] = 0u;
+    __syncthreads();
+    const float inf = __int_as_float(0x7f800000);
+    float lo[kDimMax], hi[kDimMax];
+#pragma unroll
+    for (int d = 0; d < kDimMax; ++d) { lo[d] = inf; hi[d] = -inf; }
+    unsigned int mine = 0;
+    for (int64_t i = static_cast<int64_t>(threadIdx.x) * k.stride; i < k.n; i += static_cast<int64_t>(blockDim.x) * k.stride) {
+#pragma unroll
+        for (int d = 0; d < kDimMax; ++d)
+            if (d < k.dim) {
+                const float x = k.pts[i * k.dim + d];
+                atomicAdd(&s_h[d][cell_coord(x, k.inv_cell, kSugBins - 1)], 1u);
+                lo[d] = fminf(lo[d], x);
+                hi[d] = fmaxf(hi[d], x);
+            }
+        ++mine;
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 0; d < kDimMax; ++d) {
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            lo[d] = fminf(lo[d], __shfl_xor_sync(kFull, lo[d], o));
+            hi[d] = fmaxf(hi[d], __shfl_xor_sync(kFull, hi[d], o));
+        }
+        if (lane == 0) { s_lo[d][warp] = lo[d]; s_hi[d][warp] = hi[d]; }
+    }
+    __shared__ unsigned int s_total;
+    if (threadIdx.x == 0) s_total = 0;
+    __syncthreads();
+    atomicAdd(&s_total, mine);
+    __syncthreads();
+    for (int t = threadIdx.x; t < kDimMax * kSugBins; t += blockDim.x) (&k.out->hist[0][0])[t] = (&s_h[0][0])[t];
+    if (threadIdx.x < kDimMax) {
+        float a = inf, b = -inf;
+        for (int w = 0; w < static_cast<int>(blockDim.x >> 5); ++w) { a = fminf(a, s_lo[threadIdx.x][w]); b = fmaxf(b, s_hi[threadIdx.x][w]); }
+        k.out->lo[threadIdx.x] = a;
+        k.out->hi[threadIdx.x] = b;
+    }
+    if (threadIdx.x == 0) k.out->sampled = s_total;
+}
+
+// one page-locked result block per process (the kernel writes it through its device alias), guarded by a mutex
+SuggestOut* g_suggest_host = nullptr;
+std::mutex g_suggest_mutex;
+
+int run_suggest(const float* points, int64_t n, int dim, float r, cudaStream_t st, SuggestOut* result) {
+    std::lock_guard<std::mutex> lock(g_suggest_mutex);
+    if (!g_suggest_host) CK(cudaHostAlloc(reinterpret_cast<void**>(&g_suggest_host), sizeof(SuggestOut), cudaHostAllocMapped));
+    SuggestOut* dev = nullptr;
+    CK(cudaHostGetDevicePointer(reinterpret_cast<void**>(&dev), g_suggest_host, 0));
+    SuggestArgs a;
+    a.pts = points; a.n = n; a.dim = dim;
+    a.inv_cell = 1.0f / fmaxf(r * kCellSlack, 1e-30f);
+    a.stride = n > 65536 ? n / 65536 : 1;                          // a sample of at most ~65k points
+    a.out = dev;
+    suggest_kernel<<<1, 1024, 0, st>>>(a);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
+    *result = *g_suggest_host;
+    return FRNN_OK;
+}
+
+// s(bits) of one coordinate from its 256-bin histogram
+double pair_probability(const unsigned int* h256, int bits, double total) {
+    const int m = 1 << bits;
+    double p[kSugBins];
+    for (int c = 0; c < m; ++c) p[c] = 0.0;
+    for (int c = 0; c < kSugBins; ++c) p[c & (m - 1)] += h256[c] / total;
+    if (m <= 2) return 1.0;
+    double acc = 0.0;
+    for (int c = 0; c < m; ++c) acc += p[c] * (p[(c + m - 1) & (m - 1)] + p[c] + p[(c + 1) & (m - 1)]);
+    return acc;
+}
+
+// Cost model of one event on the grid (g, bits) in microseconds of device time, fitted to the sweeps recorded in
+// DESIGN.md section 7 (B200): table entries pay for the memset and the scan, every query pays per neighbour row
+// (two table reads + bookkeeping: the 3^(g-1) term of PAPER.md:69), per candidate key tested and per survivor row
+// evaluated.  Only the ranking of the alternatives matters; the result never depends on the choice.
+struct GridCost { double us, cand, surv; };
+GridCost grid_cost(const double s[kDimMax][9], const unsigned char* order, int dim, int g, int bits, double n_event, int n_events) {
+    double cand = n_event;
+    for (int d = 0; d < g; ++d) cand *= order[d] < dim ? s[order[d]][bits] : 1.0;
+    double surv = cand;
+    for (int f = 0; f < 4; ++f)
+        if (g + f < kDim && order[g + f] < dim) surv *= s[order[g + f]][6];
+    double runs = 1.0;
+    for (int d = 0; d + 1 < g; ++d) runs *= 3.0;
+    const double entries = static_cast<double>(n_events) * pow(2.0, g * bits) * (1.0 + pow(2.0, -bits));
+    const double n_all = n_event * n_events;
+    GridCost c;
+    c.cand = cand;
+    c.surv = surv;
+    c.us = 2.0e-6 * entries + n_all * (4.9e-6 * runs * (g >= 5 ? 2.0 : 1.0) + 0.53e-6 * cand + 6.0e-6 * surv);
+    return c;
 }
 
 }  // namespace
 
 extern "C" {
 
-int frnn_version(void) { return 300; }   // 0.3.0
+int frnn_version(void) { return 400; }   // 0.4.0
 
 const char* frnn_status_string(int status) {
     switch (status) {
@@ -376,90 +723,56 @@ const char* frnn_status_string(int status) {
     }
 }
 
+const char* frnn_last_error_string(void) { return t_error; }
+
+void frnn_options_init(frnn_options* opt) {
+    if (!opt) return;
+    memset(opt, 0, sizeof(*opt));
+    opt->struct_bytes = static_cast<uint32_t>(sizeof(frnn_options));
+}
+
 size_t frnn_workspace_bytes(int64_t n_total, int n_events, int dim, int k_max) {
-    if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDimMax || k_max < 1 || n_total > 0x7fffffffll) return 0;
-    return make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim, g_order.on != 0).total;
+    return workspace_bytes_for(default_opts(), n_total, n_events, dim, k_max);
+}
+
+size_t frnn_workspace_bytes_opt(const frnn_options* opt, int64_t n_total, int n_events, int dim, int k_max) {
+    Opts o;
+    if (opts_from(opt, &o) != FRNN_OK) return 0;
+    return workspace_bytes_for(o, n_total, n_events, dim, k_max);
 }
 
 int frnn_set_grid(int grid_dims, int grid_bits) {
     if (grid_dims < 0 || grid_dims > 6 || (grid_bits != 0 && (grid_bits < 2 || grid_bits > 8))) return FRNN_ERR_INVALID_ARG;
-    g_force_dims = grid_dims;
-    g_force_bits = grid_bits;
+    std::lock_guard<std::mutex> lock(g_defaults_mutex);
+    g_defaults.grid_dims = grid_dims;
+    g_defaults.grid_bits = grid_bits;
     return FRNN_OK;
 }
 
-void frnn_get_grid(int64_t n_total, int n_events, int* grid_dims, int* grid_bits) {
-    const GridChoice g = choose_grid(n_total, n_events < 1 ? 1 : n_events);
+void frnn_get_grid(int64_t n_total, int n_events, int dim, int* grid_dims, int* grid_bits) {
+    const GridChoice g = choose_grid(default_opts(), n_total, n_events < 1 ? 1 : n_events, (dim < 1 || dim > kDimMax) ? kDim : dim);
     if (grid_dims) *grid_dims = g.dims;
     if (grid_bits) *grid_bits = g.bits;
 }
 
 int frnn_set_bin_order(const int* order, int count) {
-    if (count < 0 || count > 8 || (count > 0 && !order)) return FRNN_ERR_INVALID_ARG;
-    BinOrder o = {count > 0 ? 1 : 0, {0, 1, 2, 3, 4, 5, 6, 7}};
-    bool used[kDimMax] = {};
-    for (int k = 0; k < count; ++k) {
-        if (order[k] < 0 || order[k] >= kDimMax || used[order[k]]) return FRNN_ERR_INVALID_ARG;
-        used[order[k]] = true;
-        o.p[k] = static_cast<unsigned char>(order[k]);
-    }
-    int next = 0;
-    for (int k = count; k < 8; ++k) {                  // the rest: the unused coordinates in ascending order
-        while (used[next]) ++next;
-        used[next] = true;
-        o.p[k] = static_cast<unsigned char>(next);
-    }
-    g_order = o;
+    BinOrder o;
+    const int rc = make_order(order, count, &o);
+    if (rc != FRNN_OK) return rc;
+    std::lock_guard<std::mutex> lock(g_defaults_mutex);
+    g_defaults.order = o;
     return FRNN_OK;
 }
-
-namespace {
-// Per coordinate: the probability that two random points of the sample fall within one cell of each other
-// (cells of side r, modulo 64) = sum_c p_c (p_{c-1} + p_c + p_{c+1}).  The smaller, the more that coordinate prunes.
-constexpr int kSuggestBins = 64;
-__global__ void __launch_bounds__(1024) suggest_kernel(const float* __restrict__ pts, int64_t n, int dim, float inv_cell,
-                                                       int64_t stride, float* __restrict__ out /* kDimMax */) {
-    __shared__ unsigned int s_h[kDimMax][kSuggestBins];
-    for (int k = threadIdx.x; k < kDimMax * kSuggestBins; k += blockDim.x) (&s_h[0][0])[k] = 0u;
-    __syncthreads();
-    unsigned int mine = 0;
-    for (int64_t i = static_cast<int64_t>(threadIdx.x) * stride; i < n; i += static_cast<int64_t>(blockDim.x) * stride) {
-        for (int d = 0; d < dim; ++d) atomicAdd(&s_h[d][cell_coord(pts[i * dim + d], inv_cell, kSuggestBins - 1)], 1u);
-        ++mine;
-    }
-    __shared__ unsigned int s_total;
-    if (threadIdx.x == 0) s_total = 0;
-    __syncthreads();
-    atomicAdd(&s_total, mine);
-    __syncthreads();
-    if (threadIdx.x < kDimMax) {
-        const int d = threadIdx.x;
-        double acc = 0.0;
-        const double tot = s_total ? static_cast<double>(s_total) : 1.0;
-        for (int c = 0; c < kSuggestBins; ++c) {
-            const double pc = s_h[d][c] / tot;
-            const double nb = (s_h[d][(c + kSuggestBins - 1) % kSuggestBins] + s_h[d][c] + s_h[d][(c + 1) % kSuggestBins]) / tot;
-            acc += pc * nb;
-        }
-        out[d] = d < dim ? static_cast<float>(acc) : 2.0f;          // absent coordinates prune nothing: last
-    }
-}
-}  // namespace
 
 int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int* order, float* score, void* cuda_stream) {
     if (!points || !order || n < 1 || !(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
     if (dim < 1 || dim > kDimMax) return FRNN_ERR_UNSUPPORTED;
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    float* d_out = nullptr;
-    if (cudaMalloc(reinterpret_cast<void**>(&d_out), kDimMax * sizeof(float)) != cudaSuccess) return FRNN_ERR_CUDA;
-    const int64_t stride = n > 65536 ? n / 65536 : 1;              // a sample of at most ~65k points
-    const float inv_cell = 1.0f / fmaxf(r * kCellSlack, 1e-30f);
-    suggest_kernel<<<1, 1024, 0, st>>>(points, n, dim, inv_cell, stride, d_out);
+    SuggestOut so;
+    const int rc = run_suggest(points, n, dim, r, static_cast<cudaStream_t>(cuda_stream), &so);
+    if (rc != FRNN_OK) return rc;
     float h[kDimMax];
-    const cudaError_t e = cudaMemcpyAsync(h, d_out, sizeof(h), cudaMemcpyDeviceToHost, st);
-    const cudaError_t e2 = cudaStreamSynchronize(st);
-    cudaFree(d_out);
-    if (e != cudaSuccess || e2 != cudaSuccess) return FRNN_ERR_CUDA;
+    const double tot = so.sampled ? static_cast<double>(so.sampled) : 1.0;
+    for (int d = 0; d < kDimMax; ++d) h[d] = d < dim ? static_cast<float>(pair_probability(so.hist[d], 6, tot)) : 2.0f;   // absent coordinates prune nothing: last
     int idx[kDimMax];
     for (int d = 0; d < kDimMax; ++d) idx[d] = d;
     for (int a = 1; a < kDimMax; ++a)                               // stable insertion sort by score
@@ -469,8 +782,70 @@ int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int
     return FRNN_OK;
 }
 
+int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, float r, frnn_options* opt, frnn_grid_report* report,
+                      void* cuda_stream) {
+    if (!points || !opt || n < 1 || n_events < 1 || !(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
+    if (dim < 1 || dim > kDimMax) return FRNN_ERR_UNSUPPORTED;
+    if (opt->struct_bytes < sizeof(frnn_options)) return FRNN_ERR_INVALID_ARG;
+    SuggestOut so;
+    const int rc = run_suggest(points, n, dim, r, static_cast<cudaStream_t>(cuda_stream), &so);
+    if (rc != FRNN_OK) return rc;
+    const double tot = so.sampled ? static_cast<double>(so.sampled) : 1.0;
+    double s[kDimMax][9];
+    for (int d = 0; d < kDimMax; ++d)
+        for (int b = 0; b <= 8; ++b) s[d][b] = (d < dim && b >= 2) ? pair_probability(so.hist[d], b, tot) : 1.0;
+    // two candidate orders: the default one and the coordinates ranked by how much they prune (at the key's 64 cells)
+    unsigned char ident[8] = {0, 1, 2, 3, 4, 5, 6, 7}, ranked[8];
+    {
+        int idx[kDimMax];
+        for (int d = 0; d < kDimMax; ++d) idx[d] = d;
+        for (int a = 1; a < kDimMax; ++a)
+            for (int b = a; b > 0 && s[idx[b]][6] < s[idx[b - 1]][6]; --b) { const int t = idx[b]; idx[b] = idx[b - 1]; idx[b - 1] = t; }
+        for (int k = 0; k < 8; ++k) ranked[k] = static_cast<unsigned char>(idx[k]);
+    }
+    const double n_event = static_cast<double>(n) / n_events;
+    int ev_bits = 0;
+    while ((1ll << ev_bits) < n_events) ++ev_bits;
+    // table budget: 32 cells per point of an event (a finer table costs more to zero and scan than it saves), 2^26 in all
+    const double budget = fmin(fmax(65536.0, 32.0 * n_event), 67108864.0 / n_events);
+    struct Best { GridCost c; int g, bits; bool ok; } best[2] = {{{0, 0, 0}, 0, 0, false}, {{0, 0, 0}, 0, 0, false}};
+    for (int which = 0; which < 2; ++which) {
+        const unsigned char* ord = which ? ranked : ident;
+        for (int g = 1; g <= 6 && g <= dim; ++g)
+            for (int bits = 2; bits <= 8; ++bits) {
+                if (g * bits + ev_bits > 30 || pow(2.0, g * bits) > budget) continue;
+                const GridCost c = grid_cost(s, ord, dim, g, bits, n_event, n_events);
+                if (!best[which].ok || c.us < best[which].c.us) best[which] = Best{c, g, bits, true};
+            }
+    }
+    if (!best[0].ok) return FRNN_ERR_UNSUPPORTED;
+    const int pick = (best[1].ok && best[1].c.us < 0.9 * best[0].c.us) ? 1 : 0;     // reorder only for a clear gain: the default order is the fast path
+    opt->grid_dims = best[pick].g;
+    opt->grid_bits = best[pick].bits;
+    opt->order_count = pick ? 8 : 0;
+    for (int k = 0; k < 8; ++k) opt->order[k] = pick ? ranked[k] : k;
+    if (report) {
+        memset(report, 0, sizeof(*report));
+        report->grid_dims = best[pick].g;
+        report->grid_bits = best[pick].bits;
+        report->reordered = pick;
+        report->sampled = static_cast<int64_t>(so.sampled);
+        report->predicted_candidates = static_cast<float>(best[pick].c.cand);
+        report->predicted_survivors = static_cast<float>(best[pick].c.surv);
+        report->predicted_us = static_cast<float>(best[pick].c.us);
+        const float side = fmaxf(r * kCellSlack, 1e-30f);
+        for (int d = 0; d < kDimMax; ++d) {
+            report->extent_cells[d] = d < dim ? (so.hi[d] - so.lo[d]) / side : 0.0f;
+            report->pair_probability[d] = d < dim ? static_cast<float>(s[d][best[pick].bits]) : 1.0f;
+            report->key_probability[d] = d < dim ? static_cast<float>(s[d][6]) : 1.0f;
+        }
+    }
+    return FRNN_OK;
+}
+
 int frnn_set_graph_mode(int enabled) {
-    g_use_graph = enabled != 0;
+    std::lock_guard<std::mutex> lock(g_defaults_mutex);
+    g_defaults.use_graph = enabled != 0;
     return FRNN_OK;
 }
 
@@ -478,42 +853,46 @@ int frnn_build_ex(const float* points, int64_t n, int dim, float r, int k_max,
                   int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                   int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    return build_single(default_opts(), false, points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, out_status,
+                        out_row_ptr, workspace, workspace_bytes, cuda_stream);
+}
+
+int frnn_build_opt(const frnn_options* opt, const float* points, int64_t n, int dim, float r, int k_max,
+                   int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                   int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    Opts o;
+    const int rc = opts_from(opt, &o);
     if (rc != FRNN_OK) return rc;
-    if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
-    Call c{points, dim, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
-    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
-    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
+    return build_single(o, false, points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, out_status,
+                        out_row_ptr, workspace, workspace_bytes, cuda_stream);
 }
 
 int frnn_build_dense_ex(const float* points, int64_t n, int dim, float r, int k_max,
                         int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                         int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
                         void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
-    if (rc != FRNN_OK) return rc;
-    if (!out_count || !out_status) return FRNN_ERR_INVALID_ARG;
-    if (n > 65535ll * kDenseTile) return FRNN_ERR_UNSUPPORTED;                 // grid.y limit (8.3 M rows)
-    Call c{points, dim, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, {0, n}};
-    c.dense = true;
-    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
-    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
+    return build_single(default_opts(), true, points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, out_status,
+                        out_row_ptr, workspace, workspace_bytes, cuda_stream);
 }
 
 int frnn_build_batched(const float* points, const int64_t* event_offsets, int n_events, int dim, float r, int k_max,
                        int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                        int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
                        void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (n_events < 1 || !event_offsets || event_offsets[0] != 0) return FRNN_ERR_INVALID_ARG;
-    for (int e = 0; e < n_events; ++e)
-        if (event_offsets[e + 1] < event_offsets[e]) return FRNN_ERR_INVALID_ARG;
-    int rc = check_common(points, event_offsets[n_events], dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    return build_batched(default_opts(), points, event_offsets, n_events, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity,
+                         out_edge_offsets, out_status, out_row_ptr, workspace, workspace_bytes, cuda_stream);
+}
+
+int frnn_build_batched_opt(const frnn_options* opt, const float* points, const int64_t* event_offsets, int n_events, int dim, float r,
+                           int k_max, int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                           int64_t* out_edge_offsets, int32_t* out_status, int64_t* out_row_ptr,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    Opts o;
+    const int rc = opts_from(opt, &o);
     if (rc != FRNN_OK) return rc;
-    if (!out_edge_offsets || !out_status) return FRNN_ERR_INVALID_ARG;
-    Call c{points, dim, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets, out_status, out_row_ptr,
-           workspace, 0, 0, std::vector<int64_t>(event_offsets, event_offsets + n_events + 1)};
-    if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
-    return run_call(c, static_cast<cudaStream_t>(cuda_stream));
+    return build_batched(o, points, event_offsets, n_events, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity,
+                         out_edge_offsets, out_status, out_row_ptr, workspace, workspace_bytes, cuda_stream);
 }
 
 int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
@@ -522,14 +901,16 @@ int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
     const int64_t cap = n > 0 ? n * static_cast<int64_t>(k_max > 0 ? k_max : 0) : 0;
     int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, cap);
     if (rc != FRNN_OK) return rc;
-    const size_t need = frnn_workspace_bytes(n, 1, dim, k_max);
+    const Opts o = default_opts();
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    const size_t need = workspace_bytes_for(o, n, 1, dim, k_max);
     size_t misc_have = g_cache.misc ? 64 : 0;
     if ((rc = ensure(&g_cache.ws, &g_cache.ws_bytes, need)) != FRNN_OK) return rc;
     if ((rc = ensure(&g_cache.misc, &misc_have, 64)) != FRNN_OK) return rc;
     int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
     int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
-    rc = frnn_build_ex(points, n, dim, r, k_max, out_src, out_dst, out_d2, cap, d_count, d_status, nullptr, g_cache.ws,
-                       g_cache.ws_bytes, nullptr);       // legacy default stream, as documented
+    rc = build_single(o, false, points, n, dim, r, k_max, out_src, out_dst, out_d2, cap, d_count, d_status, nullptr, g_cache.ws,
+                      g_cache.ws_bytes, nullptr);       // legacy default stream, as documented
     if (rc != FRNN_OK) return rc;
     int32_t h_status = 0;
     CK(cudaMemcpy(out_count, d_count, 8, cudaMemcpyDeviceToHost));
@@ -540,9 +921,11 @@ int frnn_build(const float* points, int64_t n, int dim, float r, int k_max,
 int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
                     int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity, int64_t* out_count) {
     if (!out_count) return FRNN_ERR_INVALID_ARG;
-    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity);
+    int rc = check_common(points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity, true);
     if (rc != FRNN_OK) return rc;
-    const size_t need = frnn_workspace_bytes(n, 1, dim, k_max);
+    const Opts o = default_opts();
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    const size_t need = workspace_bytes_for(o, n, 1, dim, k_max);
     size_t misc_have = g_cache.misc ? 64 : 0;
     size_t edge_bytes = g_cache.edge_cap * 12;
     if ((rc = ensure_stream()) != FRNN_OK) return rc;
@@ -560,8 +943,8 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     int64_t* d_count = static_cast<int64_t*>(g_cache.misc);
     int32_t* d_status = reinterpret_cast<int32_t*>(static_cast<char*>(g_cache.misc) + 8);
     if (n > 0) CK(cudaMemcpyAsync(g_cache.pts, points, static_cast<size_t>(n) * dim * 4, cudaMemcpyHostToDevice, st));
-    rc = frnn_build_ex(static_cast<const float*>(g_cache.pts), n, dim, r, k_max, d_src, d_dst, d_d2, edge_capacity, d_count, d_status,
-                       nullptr, g_cache.ws, g_cache.ws_bytes, st);
+    rc = build_single(o, false, static_cast<const float*>(g_cache.pts), n, dim, r, k_max, d_src, d_dst, d_d2, edge_capacity, d_count, d_status,
+                      nullptr, g_cache.ws, g_cache.ws_bytes, st);
     if (rc != FRNN_OK) return rc;
     CK(cudaMemcpyAsync(out_count, d_count, 8, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -595,6 +978,7 @@ struct frnn_host_pipeline {
     int64_t n_max = 0, cap = 0;
     int k_max = 0, next = 0;
     size_t ws_bytes = 0;
+    Opts opts;                                                    // fixed at creation: the workspaces are sized for it
 };
 
 namespace {
@@ -655,14 +1039,25 @@ int pipeline_poll(frnn_host_pipeline* p) {
 }
 }  // namespace
 
-int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth, frnn_host_pipeline** out) {
+int frnn_host_pipeline_create_opt(const frnn_options* opt, int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth,
+                                  frnn_host_pipeline** out) {
     if (!out || n_max < 1 || k_max < 1 || edge_capacity < 1 || depth < 1 || depth > 16) return FRNN_ERR_INVALID_ARG;
     if (dim != kDim) return FRNN_ERR_UNSUPPORTED;
+    Opts o;
+    const int orc = opts_from(opt, &o);
+    if (orc != FRNN_OK) return orc;
     frnn_host_pipeline* p = new (std::nothrow) frnn_host_pipeline;
     if (!p) return FRNN_ERR_CUDA;
     p->n_max = n_max; p->k_max = k_max;
     p->cap = edge_capacity;
-    p->ws_bytes = frnn_workspace_bytes(n_max, 1, dim, k_max);
+    p->opts = o;
+    // events of any size up to n_max: the largest workspace over the grid classes an event of at most n_max rows can fall in
+    p->ws_bytes = 0;
+    for (int64_t n : {n_max, static_cast<int64_t>(399999), static_cast<int64_t>(16383)}) {
+        if (n > n_max) continue;
+        const size_t b = workspace_bytes_for(o, n, 1, dim, k_max);
+        if (b > p->ws_bytes) p->ws_bytes = b;
+    }
     p->slots.resize(static_cast<size_t>(depth));
     for (auto& s : p->slots) {
         bool ok = cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking) == cudaSuccess &&
@@ -673,12 +1068,16 @@ int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_ca
                   cudaMalloc(reinterpret_cast<void**>(&s.src), static_cast<size_t>(p->cap) * 12) == cudaSuccess &&
                   cudaMalloc(reinterpret_cast<void**>(&s.count), 64) == cudaSuccess &&
                   cudaMallocHost(reinterpret_cast<void**>(&s.pinned), 64) == cudaSuccess;
-        if (!ok) { cudaGetLastError(); pipeline_free(p); return FRNN_ERR_CUDA; }
+        if (!ok) { const int rc = cuda_fail(cudaGetLastError(), "frnn_host_pipeline_create"); pipeline_free(p); return rc; }
         s.dst = s.src + p->cap;
         s.d2 = reinterpret_cast<float*>(s.dst + p->cap);
     }
     *out = p;
     return FRNN_OK;
+}
+
+int frnn_host_pipeline_create(int64_t n_max, int dim, int k_max, int64_t edge_capacity, int depth, frnn_host_pipeline** out) {
+    return frnn_host_pipeline_create_opt(nullptr, n_max, dim, k_max, edge_capacity, depth, out);
 }
 
 int frnn_host_pipeline_submit(frnn_host_pipeline* p, const float* points, int64_t n, float r,
@@ -690,7 +1089,7 @@ int frnn_host_pipeline_submit(frnn_host_pipeline* p, const float* points, int64_
     if ((rc = pipeline_poll(p)) != FRNN_OK) return rc;
     CK(cudaMemcpyAsync(s.pts, points, static_cast<size_t>(n) * 32, cudaMemcpyHostToDevice, s.stream));
     int32_t* d_status = reinterpret_cast<int32_t*>(s.count + 1);
-    rc = frnn_build_ex(s.pts, n, kDim, r, p->k_max, s.src, s.dst, s.d2, p->cap, s.count, d_status, nullptr, s.ws, p->ws_bytes, s.stream);
+    rc = build_single(p->opts, false, s.pts, n, kDim, r, p->k_max, s.src, s.dst, s.d2, p->cap, s.count, d_status, nullptr, s.ws, p->ws_bytes, s.stream);
     if (rc != FRNN_OK) return rc;
     CK(cudaMemcpyAsync(s.pinned, s.count, 12, cudaMemcpyDeviceToHost, s.stream));
     CK(cudaEventRecord(s.built, s.stream));
@@ -715,11 +1114,13 @@ void frnn_host_pipeline_destroy(frnn_host_pipeline* p) {
 int frnn_last_launch_count(void) { return t_launches; }
 
 int frnn_set_profiling(int enabled) {
-    g_timeline = enabled == 2;
+    {
+        std::lock_guard<std::mutex> lock(g_defaults_mutex);
+        g_defaults.timeline = enabled == 2;
+    }
     if (enabled == 2) enabled = 0;
     if (enabled && !g_ev_valid) {
-        for (int i = 0; i <= kPhases; ++i)
-            if (cudaEventCreate(&g_ev[i]) != cudaSuccess) return FRNN_ERR_CUDA;
+        for (int i = 0; i <= kPhases; ++i) CK(cudaEventCreate(&g_ev[i]));
         g_ev_valid = true;
     }
     g_profiling = enabled != 0;
@@ -728,19 +1129,18 @@ int frnn_set_profiling(int enabled) {
 
 int frnn_get_profile(float* phase_ms, int max_phases) {
     if (!g_ev_valid || !phase_ms) return FRNN_ERR_INVALID_ARG;
-    if (cudaEventSynchronize(g_ev[kPhases]) != cudaSuccess) return FRNN_ERR_CUDA;
+    CK(cudaEventSynchronize(g_ev[kPhases]));
     const int n = max_phases < kPhases ? max_phases : kPhases;
-    for (int i = 0; i < n; ++i)
-        if (cudaEventElapsedTime(&phase_ms[i], g_ev[i], g_ev[i + 1]) != cudaSuccess) return FRNN_ERR_CUDA;
+    for (int i = 0; i < n; ++i) CK(cudaEventElapsedTime(&phase_ms[i], g_ev[i], g_ev[i + 1]));
     return n;
 }
 
 int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, int dim, double* begin_us, double* end_us, int max_phases) {
     if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1 || dim < 1 || dim > kDimMax) return FRNN_ERR_INVALID_ARG;
-    const Layout L = make_layout(n_total, n_events, choose_grid(n_total, n_events, dim), dim, g_order.on != 0);
+    const Opts o = default_opts();
+    const Layout L = make_layout(n_total, n_events, choose_grid(o, n_total, n_events, dim), dim, o.order.on != 0);
     unsigned long long h[2 * kTimelinePhases];
-    if (cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess)
-        return FRNN_ERR_CUDA;
+    CK(cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost));
     const int n = max_phases < kTimelinePhases ? max_phases : kTimelinePhases;
     const unsigned long long t0 = ~h[0];                   // start of the first kernel
     for (int i = 0; i < n; ++i) {
@@ -756,10 +1156,10 @@ const char* frnn_phase_name(int phase) { return (phase >= 0 && phase < kPhases) 
 
 void frnn_release_cached(void) {
     {
-        std::lock_guard<std::mutex> lock(g_graph_mutex);
-        for (auto& g : g_graphs) cudaGraphExecDestroy(g.exec);
-        g_graphs.clear();
+        std::lock_guard<std::mutex> lock(g_exec_mutex);
+        g_execs.clear();
     }
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
     if (g_cache.ws) cudaFree(g_cache.ws);
     if (g_cache.misc) cudaFree(g_cache.misc);
     if (g_cache.pts) cudaFree(g_cache.pts);

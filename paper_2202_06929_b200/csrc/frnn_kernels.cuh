@@ -202,67 +202,92 @@ __device__ __forceinline__ int event_of_row(const int64_t* __restrict__ ev_off, 
 // Host event offsets travel as kernel arguments, kN at a time.
 struct OffsetChunk {
     static constexpr int kN = 128;
+    int64_t* ev_off;
     int first, count;
     int64_t v[kN];
 };
-__global__ void set_offsets_kernel(OffsetChunk c, int64_t* __restrict__ ev_off) {
-    if (static_cast<int>(threadIdx.x) < c.count) ev_off[c.first + threadIdx.x] = c.v[threadIdx.x];
+__global__ void set_offsets_kernel(OffsetChunk c) {
+    if (static_cast<int>(threadIdx.x) < c.count) c.ev_off[c.first + threadIdx.x] = c.v[threadIdx.x];
 }
 
 // ------------------------------------------------------------------------------------------------
 // S2: cell index + histogram.  The atomicAdd's return value is the point's rank inside its cell,
 // which makes the later scatter a pure function of (cell_start, rank): no second atomic pass.
 // ------------------------------------------------------------------------------------------------
+// Every kernel of the path takes ONE by-value argument struct: a call is then a list of (function, grid, struct)
+// records, which the host either launches one by one or writes into the kernel nodes of a cached CUDA graph
+// (cudaGraphExecKernelNodeSetParams) -- the graph does not depend on n, the pointers or the parameters of a call.
+struct BinArgs {
+    const float* pts;
+    int dim;
+    int64_t n_total;
+    const int64_t* ev_off;
+    int n_events;
+    float inv_cell;
+    int bits;
+    uint32_t* cell_count;
+    uint32_t* pcell;
+    uint32_t* prank;
+    BinOrder order;
+    unsigned long long* stamps;
+};
 template <int G>
-__global__ void __launch_bounds__(256) bin_kernel(const float* __restrict__ pts, int dim, int64_t n_total,
-                                                  const int64_t* __restrict__ ev_off, int n_events,
-                                                  float inv_cell, int bits,
-                                                  uint32_t* __restrict__ cell_count,
-                                                  uint32_t* __restrict__ pcell, uint32_t* __restrict__ prank,
-                                                  BinOrder order, unsigned long long* stamps) {
-    stamp_begin(stamps, 0);
+__global__ void __launch_bounds__(256) bin_kernel(BinArgs k) {
+    stamp_begin(k.stamps, 0);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < n_total) {
+    if (i < k.n_total) {
         float4 a, b;
-        load_point(pts, i, dim, a, b);
-        const uint32_t ev = ev_off ? static_cast<uint32_t>(event_of_row(ev_off, n_events, i)) : 0u;
-        const uint32_t lin = order.on ? cell_ordered<G>(pts + i * dim, dim, ev, inv_cell, bits, order) : cell_of_point<G>(a, b, ev, inv_cell, bits);
-        pcell[i] = lin;
-        prank[i] = atomicAdd(&cell_count[padded(lin, bits)], 1u);
+        load_point(k.pts, i, k.dim, a, b);
+        const uint32_t ev = k.ev_off ? static_cast<uint32_t>(event_of_row(k.ev_off, k.n_events, i)) : 0u;
+        const uint32_t lin = k.order.on ? cell_ordered<G>(k.pts + i * k.dim, k.dim, ev, k.inv_cell, k.bits, k.order)
+                                        : cell_of_point<G>(a, b, ev, k.inv_cell, k.bits);
+        k.pcell[i] = lin;
+        k.prank[i] = atomicAdd(&k.cell_count[padded(lin, k.bits)], 1u);
     }
-    stamp_end(stamps, 0);
+    stamp_end(k.stamps, 0);
 }
 
 // ------------------------------------------------------------------------------------------------
 // S4: counting-sort scatter.  Order inside a cell is the (arbitrary) atomic order; the final
 // result does not depend on it because every row is ordered by dst at the end.
 // ------------------------------------------------------------------------------------------------
+struct ScatterArgs {
+    const float* pts;
+    int dim;
+    int64_t n_total;
+    int bits;
+    float inv_cell;
+    const uint32_t* cell_start;
+    const uint32_t* pcell;
+    const uint32_t* prank;
+    float4* spts;
+    int32_t* sidx;
+    uint32_t* skey;
+    float4* spts_hi;
+    uint32_t* scell;
+    BinOrder order;
+    unsigned long long* stamps;
+};
 template <int G>
-__global__ void __launch_bounds__(256) scatter_kernel(const float* __restrict__ pts, int dim, int64_t n_total, int bits, float inv_cell,
-                                                      const uint32_t* __restrict__ cell_start,
-                                                      const uint32_t* __restrict__ pcell,
-                                                      const uint32_t* __restrict__ prank,
-                                                      float4* __restrict__ spts, int32_t* __restrict__ sidx,
-                                                      uint32_t* __restrict__ skey, float4* __restrict__ spts_hi,
-                                                      uint32_t* __restrict__ scell, BinOrder order, unsigned long long* stamps) {
-    stamp_begin(stamps, 2);
+__global__ void __launch_bounds__(256) scatter_kernel(ScatterArgs k) {
+    stamp_begin(k.stamps, 2);
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < n_total) {
-        const uint32_t lin = pcell[i];
-        const uint32_t s = cell_start[padded(lin, bits)] + prank[i];
-        if (scell) scell[s] = lin;                                 // a bin order is set: the search cannot recompute the cell from the row
+    if (i < k.n_total) {
+        const uint32_t lin = k.pcell[i];
+        const uint32_t s = k.cell_start[padded(lin, k.bits)] + k.prank[i];
+        if (k.scell) k.scell[s] = lin;                             // a bin order is set: the search cannot recompute the cell from the row
         float4 a, b;
-        load_point(pts, i, dim, a, b);
-        store_row(spts + 2 * static_cast<int64_t>(s), a, b);      // one 32-byte sector, one transaction
-        sidx[s] = static_cast<int32_t>(i);
-        skey[s] = order.on ? key_ordered<G>(pts + i * dim, dim, inv_cell, order) : key_of_point<G>(a, b, inv_cell);
-        if (spts_hi) {                                             // dim > 8: coordinates 8..15 travel in a second row
+        load_point(k.pts, i, k.dim, a, b);
+        store_row(k.spts + 2 * static_cast<int64_t>(s), a, b);    // one 32-byte sector, one transaction
+        k.sidx[s] = static_cast<int32_t>(i);
+        k.skey[s] = k.order.on ? key_ordered<G>(k.pts + i * k.dim, k.dim, k.inv_cell, k.order) : key_of_point<G>(a, b, k.inv_cell);
+        if (k.spts_hi) {                                           // dim > 8: coordinates 8..15 travel in a second row
             float4 c, d;
-            load_point_hi(pts, i, dim, c, d);
-            store_row(spts_hi + 2 * static_cast<int64_t>(s), c, d);
+            load_point_hi(k.pts, i, k.dim, c, d);
+            store_row(k.spts_hi + 2 * static_cast<int64_t>(s), c, d);
         }
     }
-    stamp_end(stamps, 2);
+    stamp_end(k.stamps, 2);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -277,9 +302,20 @@ constexpr int kCellTile = 4 * kCellThreads;      // table entries per block (upp
 
 // A block owns `rows_per_block` whole padded rows = rows_per_block * (2^bits + 1) <= kCellTile
 // entries (a multiple of 4, so every thread moves one aligned uint4).
-__global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(uint32_t* __restrict__ cells, int64_t n_entries, int rows_per_block,
-                                                                 int bits, unsigned int* __restrict__ cursor,
-                                                                 unsigned long long* stamps) {
+struct ScanArgs {
+    uint32_t* cells;
+    int64_t n_entries;
+    int rows_per_block;
+    int bits;
+    unsigned int* cursor;
+    unsigned long long* stamps;
+};
+__global__ void __launch_bounds__(kCellThreads) cell_scan_kernel(ScanArgs k) {
+    uint32_t* __restrict__ cells = k.cells;
+    const int64_t n_entries = k.n_entries;
+    const int rows_per_block = k.rows_per_block, bits = k.bits;
+    unsigned int* __restrict__ cursor = k.cursor;
+    unsigned long long* stamps = k.stamps;
     stamp_begin(stamps, 1);
     __shared__ uint32_t s_pts[32];
     __shared__ uint32_t s_base;
@@ -838,8 +874,15 @@ __global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
 // quadratic in the number of tiles).  Calls with few tiles skip this kernel: one dependent launch less.
 // ------------------------------------------------------------------------------------------------
 constexpr int kPrefixThreads = 1024;
-__global__ void __launch_bounds__(kPrefixThreads) tile_prefix_kernel(const unsigned long long* __restrict__ tile_deg, uint32_t n_tiles,
-                                                                     unsigned long long* __restrict__ tile_prefix) {
+struct PrefixArgs {
+    const unsigned long long* tile_deg;
+    uint32_t n_tiles;
+    unsigned long long* tile_prefix;
+};
+__global__ void __launch_bounds__(kPrefixThreads) tile_prefix_kernel(PrefixArgs k) {
+    const unsigned long long* __restrict__ tile_deg = k.tile_deg;
+    const uint32_t n_tiles = k.n_tiles;
+    unsigned long long* __restrict__ tile_prefix = k.tile_prefix;
     __shared__ unsigned long long s_w[kPrefixThreads / 32];
     __shared__ unsigned long long s_carry;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -879,13 +922,24 @@ __global__ void __launch_bounds__(kPrefixThreads) tile_prefix_kernel(const unsig
 
 // ------------------------------------------------------------------------------------------------
 // S8-S10: emit.  Thread per row in ORIGINAL order.  The search pass left sum(min(|S_i|, k_max)) per
-// 512-row tile in tile_deg, so a block gets its global edge offset by summing the totals of the
-// tiles before it (no inter-block wait), scans its own capped degrees -> CSR row_ptr, and every row
-// places its hits at row_ptr[i] + (rank of dst among the row's hits): no sort, the COO comes out
-// (src,dst)-sorted.  Rows whose hits did not fit the slot buffer, or with more than k_max hits, are
-// recomputed by the whole warp: exact K-smallest by (d2, j) through bisection on the bit pattern of
-// d2 and then on j among ties (storage-free), hits written unsorted, ordered by a bitonic network.
+// 256-row tile in tile_deg, so a block gets its global edge offset by summing the totals of the
+// tiles before it (no inter-block wait), scans its own capped degrees -> CSR row_ptr, and then
+// resolves its rows by class (c = |S_i|, the uncapped count; K = k_max; kSlot = 32 hit slots per row):
+//   small   c <= K, c <= kSlot   one thread per OUTPUT EDGE: position = rank of dst among the row's stored hits
+//   medium  K < c <= kSlot       (S8 from the slot buffer, no recomputation) one thread per STORED HIT: its rank
+//                                under (d2, j) among the row's hits decides whether it is kept (rank < K); a second
+//                                sweep places the kept hits by dst among the kept
+//   big     c > kSlot            the slot buffer overflowed: the row is recomputed by a whole warp, ONE pass over
+//                                its neighbourhood collecting the in-radius hits as 64-bit keys (d2 bits, j) into
+//                                the warp's staging buffer in shared memory (kStage entries); if c > K a bitonic
+//                                sort of the keys keeps the K smallest (north_star (3): warp-level bitonic top-K
+//                                on (d2, index) with index tie-break), a second sort orders the kept by dst
+//   huge    c > kStage           beyond the staging capacity: threshold by storage-free bisection on the bit
+//                                pattern of d2 and then on j among ties (one neighbourhood pass per step), hits
+//                                written unsorted and ordered in place by a bitonic network in global memory
 // ------------------------------------------------------------------------------------------------
+constexpr int kStage = 512;            // staging entries per warp for recomputed rows (K <= 512: 16 keys per lane)
+
 __device__ __forceinline__ void cmp_swap(int32_t* dst, float* d2, int64_t lo, int64_t hi) {
     const int32_t x = dst[lo], y = dst[hi];
     if (x > y) {
@@ -918,6 +972,23 @@ __device__ __forceinline__ void warp_sort_rows(int32_t* dst, float* d2, int64_t 
     }
 }
 
+// ascending bitonic sort of the 64-bit keys k[0..p2) in shared memory by one warp; p2 a power of two >= 2, entries
+// beyond the data preset to ~0 (keys are < 2^63, so the padding stays at the top)
+__device__ __forceinline__ void warp_sort_keys(unsigned long long* k, int p2, int lane) {
+    for (int size = 2; size <= p2; size <<= 1) {
+        for (int stride = size >> 1; stride >= 1; stride >>= 1) {
+            for (int t = lane; t < (p2 >> 1); t += 32) {
+                const int lo = ((t & ~(stride - 1)) << 1) | (t & (stride - 1));
+                const int hi = lo | stride;
+                const unsigned long long x = k[lo], y = k[hi];
+                const bool up = (lo & size) == 0;
+                if ((x > y) == up) { k[lo] = y; k[hi] = x; }
+            }
+            __syncwarp();
+        }
+    }
+}
+
 struct EmitArgs {
     const float* pts;             // original points (to recompute the cell of a big row), n x dim
     int dim;
@@ -944,14 +1015,15 @@ struct EmitArgs {
     float r2, inv_cell;
     int bits;
     uint32_t k_max;
+    uint32_t n_tiles;             // number of emit tiles (= the launch grid unless the grid was rounded up)
     int dense;                    // 1: no grid exists (frnn_build_dense_ex): recomputed rows scan their whole event
     BinOrder order;
 };
 
 template <int G, bool INTERIOR>
 __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int64_t row_rp, int64_t row_ev, uint32_t row_cnt,
-                                             uint32_t cell, const float4& qa, const float4& qb, int* s_delta, int lane,
-                                             int lane_delta, uint32_t lt_mask) {
+                                          uint32_t cell, const float4& qa, const float4& qb, int* s_delta,
+                                          unsigned long long* stage, int lane, int lane_delta, uint32_t lt_mask) {
     const float inf = __int_as_float(0x7f800000);
     const bool hi = a.dim > kDim;                         // coordinates 8..15 exist: the chain goes on over them
     float4 qc = make_float4(0.f, 0.f, 0.f, 0.f), qd = qc;
@@ -991,8 +1063,55 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
             g(d2 <= a.r2 && cj != static_cast<int32_t>(row), cj, d2);
         });
     };
-    // threshold key (dthr, jthr): keep hits with (d2 bits, j) <= it.  d2 >= +0 always (the chain
-    // starts at +0 and adds squares), so bit patterns order like values.
+    const int32_t src = static_cast<int32_t>(row - row_ev);
+    const uint32_t kept = row_cnt < a.k_max ? row_cnt : a.k_max;
+
+    if (row_cnt <= static_cast<uint32_t>(kStage)) {
+        // ---- ONE pass: every in-radius hit becomes a key (d2 bits << 32 | j) in the staging buffer.  d2 >= +0 always
+        // (the chain starts at +0 and adds squares), so bit patterns order like values and the key order IS (d2, j).
+        uint32_t off = 0;
+        visit([&](bool in, int32_t cj, float d2) {
+            const uint32_t m = __ballot_sync(kFull, in);
+            if (in) {
+                const uint32_t at = off + __popc(m & lt_mask);
+                if (at < static_cast<uint32_t>(kStage))
+                    stage[at] = (static_cast<unsigned long long>(__float_as_uint(d2)) << 32) | static_cast<uint32_t>(cj);
+            }
+            off += __popc(m);
+        });
+        uint32_t len = off < static_cast<uint32_t>(kStage) ? off : static_cast<uint32_t>(kStage);    // == row_cnt
+        __syncwarp();
+        if (len > a.k_max) {                              // S8: the K smallest keys
+            int p2 = 2;
+            while (static_cast<uint32_t>(p2) < len) p2 <<= 1;
+            for (int t = static_cast<int>(len) + lane; t < p2; t += 32) stage[t] = ~0ull;
+            __syncwarp();
+            warp_sort_keys(stage, p2, lane);
+            len = a.k_max;
+        }
+        // ---- order the kept hits by dst: keys (j << 32 | d2 bits), second sort
+        int p2 = 2;
+        while (static_cast<uint32_t>(p2) < len) p2 <<= 1;
+        for (int t = lane; t < p2; t += 32) {
+            const unsigned long long v = stage[t];
+            stage[t] = static_cast<uint32_t>(t) < len ? ((v << 32) | (v >> 32)) : ~0ull;
+        }
+        __syncwarp();
+        warp_sort_keys(stage, p2, lane);
+        for (uint32_t t = lane; t < len; t += 32) {       // coalesced stores
+            const unsigned long long v = stage[t];
+            const int64_t pos = row_rp + t;
+            if (pos < a.capacity) {
+                a.out_src[pos] = src;
+                a.out_dst[pos] = static_cast<int32_t>(v >> 32) - static_cast<int32_t>(row_ev);
+                a.out_d2[pos] = __uint_as_float(static_cast<uint32_t>(v));
+            }
+        }
+        __syncwarp();
+        return;
+    }
+
+    // ---- beyond the staging capacity.  Threshold key (dthr, jthr): keep hits with (d2 bits, j) <= it.
     uint32_t dthr = __float_as_uint(a.r2);
     int32_t jthr = 0x7fffffff;
     if (row_cnt > a.k_max) {
@@ -1017,7 +1136,6 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
         dthr = dlo;
         jthr = jlo;
     }
-    const int32_t src = static_cast<int32_t>(row - row_ev);
     uint32_t off = 0;
     visit([&](bool in, int32_t cj, float d2) {
         const uint32_t db = __float_as_uint(d2);
@@ -1030,8 +1148,7 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
         off += __popc(m);
     });
     __syncwarp();
-    const int64_t kept = row_cnt < a.k_max ? row_cnt : a.k_max;
-    if (row_rp + kept <= a.capacity)                       // rows cut by the capacity stay unsorted
+    if (row_rp + static_cast<int64_t>(kept) <= a.capacity)   // rows cut by the capacity stay unsorted
         warp_sort_rows(a.out_dst + row_rp, a.out_d2 + row_rp, kept, lane);
     __syncwarp();
 }
@@ -1042,12 +1159,17 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     __shared__ unsigned long long s_warp[kEmitThreads / 32];
     __shared__ unsigned long long s_prefix;
     __shared__ int32_t s_evb[kEmitThreads];                // first row of the event of every row (batched calls)
-    __shared__ uint32_t s_bigmask[kEmitThreads / 32];
+    __shared__ uint32_t s_bigmask[kEmitThreads / 32];      // rows that the edge-parallel sweep skips (medium, big, huge)
     __shared__ int s_delta[kEmitThreads / 32][32];
+    __shared__ uint32_t s_mp[kEmitThreads + 1];            // medium rows: offsets of their STORED hits inside the tile
+    __shared__ uint32_t s_kept[kEmitThreads];              // medium rows: bit h set = stored hit h is among the K nearest
+    __shared__ uint32_t s_mwarp[kEmitThreads / 32];
+    __shared__ unsigned long long s_stage[kEmitThreads / 32][kStage];   // big rows: per-warp staging of (d2, j) keys
     stamp_begin(a.stamps, 4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t tile = blockIdx.x;
+    if (tile >= a.n_tiles) { stamp_end(a.stamps, 4); return; }
     const int64_t tile_row0 = static_cast<int64_t>(tile) * kEmitThreads;
     const int64_t i = tile_row0 + threadIdx.x;
     const bool has = i < a.n_total;
@@ -1058,7 +1180,7 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     for (uint32_t t = threadIdx.x; t < (a.tile_prefix ? 0u : tile); t += kEmitThreads) {
         unsigned long long part[kDegSlices];
 #pragma unroll
-        for (int sl = 0; sl < kDegSlices; ++sl) part[sl] = a.tile_deg[static_cast<size_t>(sl) * gridDim.x + t];      // all in flight
+        for (int sl = 0; sl < kDegSlices; ++sl) part[sl] = a.tile_deg[static_cast<size_t>(sl) * a.n_tiles + t];      // all in flight
 #pragma unroll
         for (int sl = 0; sl < kDegSlices; ++sl) before += part[sl];
     }
@@ -1088,11 +1210,13 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     const unsigned long long local_rp = wexcl + (incl - deg);
     const unsigned long long tile_base = s_prefix;
     const int64_t rp = static_cast<int64_t>(tile_base + local_rp);                 // row_ptr[i]
-    const bool big = has && (c > kSlot || c > a.k_max);
+    const bool big = has && c > kSlot;                     // recomputed by a whole warp
+    const bool medium = has && c > a.k_max && c <= kSlot;  // K-cap selection from the slot buffer
     s_rp[threadIdx.x] = local_rp;
     if (threadIdx.x == kEmitThreads - 1) s_rp[kEmitThreads] = local_rp + deg;
     const uint32_t bigs_warp = __ballot_sync(kFull, big);
-    if (lane == 0) s_bigmask[warp] = bigs_warp;
+    const uint32_t skip_warp = __ballot_sync(kFull, big || medium);
+    if (lane == 0) s_bigmask[warp] = skip_warp;
     // ---- CSR offsets, count, status, per-event edge offsets
     int64_t ev_base = 0;
     if (has) {
@@ -1113,6 +1237,25 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
         }
     }
     s_evb[threadIdx.x] = static_cast<int32_t>(ev_base);
+    // medium rows exist only when K < kSlot (block-uniform test first: the usual K costs nothing here)
+    const bool any_medium = a.k_max < static_cast<uint32_t>(kSlot) && __syncthreads_or(medium ? 1 : 0) != 0;
+    if (any_medium) {                                      // block scan of the stored-hit counts of the medium rows
+        const uint32_t mc = medium ? c : 0u;
+        uint32_t mi = mc;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(kFull, mi, o);
+            if (lane >= o) mi += t;
+        }
+        if (lane == 31) s_mwarp[warp] = mi;
+        s_kept[threadIdx.x] = 0u;
+        __syncthreads();
+        uint32_t mexcl = 0;
+#pragma unroll
+        for (int w = 0; w < kEmitThreads / 32; ++w) mexcl += (w < warp) ? s_mwarp[w] : 0u;
+        s_mp[threadIdx.x] = mexcl + (mi - mc);
+        if (threadIdx.x == kEmitThreads - 1) s_mp[kEmitThreads] = mexcl + mi;
+    }
     __syncthreads();
     // ---- rows that fit their slot buffer, ONE THREAD PER OUTPUT EDGE: edge p of the tile belongs to the row r
     // with s_rp[r] <= p < s_rp[r+1] (binary search in shared memory), is the row's hit number m = p - s_rp[r],
@@ -1123,9 +1266,9 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
 #pragma unroll
         for (int step = kEmitThreads / 2; step >= 1; step >>= 1)
             if (s_rp[r + step] <= p) r += step;
-        if ((s_bigmask[r >> 5] >> (r & 31)) & 1u) continue;            // resolved below by a whole warp
+        if ((s_bigmask[r >> 5] >> (r & 31)) & 1u) continue;            // medium / big: resolved below
         const unsigned long long r0 = s_rp[r];
-        const uint32_t cr = static_cast<uint32_t>(s_rp[r + 1] - r0);   // = uncapped count (the row is not big)
+        const uint32_t cr = static_cast<uint32_t>(s_rp[r + 1] - r0);   // = uncapped count (the row is small)
         const uint32_t m = static_cast<uint32_t>(p - r0);
         const int64_t row = tile_row0 + r;
         const int2* h = a.hits + row * kSlot;
@@ -1143,6 +1286,52 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
             a.out_src[pos] = static_cast<int32_t>(row) - eb;
             a.out_dst[pos] = mine.x - eb;
             a.out_d2[pos] = __int_as_float(mine.y);
+        }
+    }
+    // ---- medium rows (K < c <= kSlot): S8 from the slot buffer, ONE THREAD PER STORED HIT.  Sweep 1: the rank of my hit
+    // under (d2 bits, j) among the row's c hits (keys are distinct: j is); rank < K = kept, noted as a bit of the row's
+    // word.  Sweep 2: a kept hit goes to position (number of kept hits of the row with a smaller dst).
+    if (any_medium) {
+        const uint32_t med_total = s_mp[kEmitThreads];
+        for (int sweep = 0; sweep < 2; ++sweep) {
+            for (uint32_t q = threadIdx.x; q < med_total; q += kEmitThreads) {
+                int r = 0;
+#pragma unroll
+                for (int step = kEmitThreads / 2; step >= 1; step >>= 1)
+                    if (s_mp[r + step] <= q) r += step;
+                const uint32_t hnum = q - s_mp[r];
+                const uint32_t cr = s_mp[r + 1] - s_mp[r];
+                const int64_t row = tile_row0 + r;
+                const int2* h = a.hits + row * kSlot;
+                const int2 mine = h[hnum];
+                if (sweep == 0) {
+                    const unsigned long long mykey = (static_cast<unsigned long long>(static_cast<uint32_t>(mine.y)) << 32) | static_cast<uint32_t>(mine.x);
+                    uint32_t rank = 0;
+                    for (uint32_t u = 0; u < cr; u += 2) {             // two hits per 16-byte load (slot buffer padded to kSlot)
+                        const int4 v = *reinterpret_cast<const int4*>(h + u);
+                        const unsigned long long k0 = (static_cast<unsigned long long>(static_cast<uint32_t>(v.y)) << 32) | static_cast<uint32_t>(v.x);
+                        const unsigned long long k1 = (static_cast<unsigned long long>(static_cast<uint32_t>(v.w)) << 32) | static_cast<uint32_t>(v.z);
+                        rank += (k0 < mykey) + (u + 1 < cr && k1 < mykey);
+                    }
+                    if (rank < a.k_max) atomicOr(&s_kept[r], 1u << hnum);
+                } else {
+                    const uint32_t kept = s_kept[r];
+                    if (!((kept >> hnum) & 1u)) continue;
+                    uint32_t rank = 0;
+                    for (uint32_t u = 0; u < cr; u += 2) {
+                        const int4 v = *reinterpret_cast<const int4*>(h + u);
+                        rank += (((kept >> u) & 1u) && v.x < mine.x) + (((kept >> (u + 1)) & 1u) && v.z < mine.x);
+                    }
+                    const int64_t pos = static_cast<int64_t>(tile_base + s_rp[r]) + rank;
+                    if (pos < a.capacity) {
+                        const int32_t eb = s_evb[r];
+                        a.out_src[pos] = static_cast<int32_t>(row) - eb;
+                        a.out_dst[pos] = mine.x - eb;
+                        a.out_d2[pos] = __int_as_float(mine.y);
+                    }
+                }
+            }
+            __syncthreads();
         }
     }
     // ---- big rows: recompute with the whole warp
@@ -1168,8 +1357,8 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
                 const uint32_t cd = (cell >> (d * a.bits)) & mask;
                 interior = interior && cd != 0u && cd != mask;
             }
-            if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
-            else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], lane, lane_delta, lt_mask);
+            if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], lane, lane_delta, lt_mask);
+            else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], lane, lane_delta, lt_mask);
         }
     }
     stamp_end(a.stamps, 4);

@@ -22,26 +22,49 @@ FRNN_ERR_WORKSPACE = -4
 FRNN_ERR_CUDA = -5
 
 _c = ctypes
+
+
+class FrnnOptions(_c.Structure):
+    """``frnn_options`` of include/frnn.h (per-call grid / bin order / launch mode)."""
+    _fields_ = [("struct_bytes", _c.c_uint32), ("grid_dims", _c.c_int32), ("grid_bits", _c.c_int32), ("order_count", _c.c_int32),
+                ("order", _c.c_int32 * 8), ("launch_mode", _c.c_int32), ("timeline", _c.c_int32), ("reserved", _c.c_int32 * 4)]
+
+
+class FrnnGridReport(_c.Structure):
+    """``frnn_grid_report`` of include/frnn.h (what frnn_suggest_grid saw and predicts)."""
+    _fields_ = [("grid_dims", _c.c_int32), ("grid_bits", _c.c_int32), ("reordered", _c.c_int32), ("sampled", _c.c_int64),
+                ("predicted_candidates", _c.c_float), ("predicted_survivors", _c.c_float), ("predicted_us", _c.c_float),
+                ("extent_cells", _c.c_float * 16), ("pair_probability", _c.c_float * 16), ("key_probability", _c.c_float * 16)]
+
+
+FRNN_LAUNCH_DEFAULT, FRNN_LAUNCH_GRAPH, FRNN_LAUNCH_PLAIN = 0, 1, 2
+_OPT = _c.POINTER(FrnnOptions)
+_BUILD_ARGS = [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
+               _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
+               _c.c_void_p, _c.c_void_p, _c.c_void_p,
+               _c.c_void_p, _c.c_size_t, _c.c_void_p]
+_BATCHED_ARGS = [_c.c_void_p, _c.POINTER(_c.c_int64), _c.c_int, _c.c_int, _c.c_float, _c.c_int,
+                 _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
+                 _c.c_void_p, _c.c_void_p, _c.c_void_p,
+                 _c.c_void_p, _c.c_size_t, _c.c_void_p]
 _SIGNATURES = {
     "frnn_version": (_c.c_int, []),
     "frnn_status_string": (_c.c_char_p, [_c.c_int]),
+    "frnn_last_error_string": (_c.c_char_p, []),
+    "frnn_options_init": (None, [_OPT]),
     "frnn_workspace_bytes": (_c.c_size_t, [_c.c_int64, _c.c_int, _c.c_int, _c.c_int]),
+    "frnn_workspace_bytes_opt": (_c.c_size_t, [_OPT, _c.c_int64, _c.c_int, _c.c_int, _c.c_int]),
     "frnn_set_grid": (_c.c_int, [_c.c_int, _c.c_int]),
-    "frnn_get_grid": (None, [_c.c_int64, _c.c_int, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int)]),
+    "frnn_get_grid": (None, [_c.c_int64, _c.c_int, _c.c_int, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int)]),
+    "frnn_suggest_grid": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_int, _c.c_float, _OPT, _c.POINTER(FrnnGridReport), _c.c_void_p]),
+    "frnn_build_opt": (_c.c_int, [_OPT] + _BUILD_ARGS),
+    "frnn_build_batched_opt": (_c.c_int, [_OPT] + _BATCHED_ARGS),
+    "frnn_host_pipeline_create_opt": (_c.c_int, [_OPT, _c.c_int64, _c.c_int, _c.c_int, _c.c_int64, _c.c_int, _c.POINTER(_c.c_void_p)]),
     "frnn_build": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
                               _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.POINTER(_c.c_int64)]),
-    "frnn_build_ex": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
-                                 _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
-                                 _c.c_void_p, _c.c_void_p, _c.c_void_p,
-                                 _c.c_void_p, _c.c_size_t, _c.c_void_p]),
-    "frnn_build_dense_ex": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
-                                       _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
-                                       _c.c_void_p, _c.c_void_p, _c.c_void_p,
-                                       _c.c_void_p, _c.c_size_t, _c.c_void_p]),
-    "frnn_build_batched": (_c.c_int, [_c.c_void_p, _c.POINTER(_c.c_int64), _c.c_int, _c.c_int, _c.c_float, _c.c_int,
-                                      _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,
-                                      _c.c_void_p, _c.c_void_p, _c.c_void_p,
-                                      _c.c_void_p, _c.c_size_t, _c.c_void_p]),
+    "frnn_build_ex": (_c.c_int, _BUILD_ARGS),
+    "frnn_build_dense_ex": (_c.c_int, _BUILD_ARGS),
+    "frnn_build_batched": (_c.c_int, _BATCHED_ARGS),
     "frnn_build_host": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
                                    _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64, _c.POINTER(_c.c_int64)]),
     "frnn_last_launch_count": (_c.c_int, []),
@@ -92,7 +115,8 @@ def lib() -> ctypes.CDLL:
 class FrnnError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
-        super().__init__(f"{where}: {frnn_status_string(status)} ({status})")
+        detail = f" [{frnn_last_error_string()}]" if status == FRNN_ERR_CUDA else ""
+        super().__init__(f"{where}: {frnn_status_string(status)} ({status}){detail}")
 
 
 def _check(status: int, where: str):
@@ -108,7 +132,30 @@ def frnn_status_string(status: int) -> str:
     return lib().frnn_status_string(int(status)).decode()
 
 
-def frnn_workspace_bytes(n_total: int, n_events: int = 1, dim: int = 8, k_max: int = 1) -> int:
+def frnn_last_error_string() -> str:
+    return lib().frnn_last_error_string().decode()
+
+
+def frnn_options(grid_dims: int = 0, grid_bits: int = 0, order=None, launch_mode: int = FRNN_LAUNCH_DEFAULT,
+                 timeline: bool = False) -> FrnnOptions:
+    """An initialised ``frnn_options`` (frnn_options_init + the given fields)."""
+    o = FrnnOptions()
+    lib().frnn_options_init(_c.byref(o))
+    o.grid_dims, o.grid_bits, o.launch_mode, o.timeline = int(grid_dims), int(grid_bits), int(launch_mode), int(bool(timeline))
+    order = [int(v) for v in (order or [])]
+    o.order_count = len(order)
+    for k, v in enumerate(order):
+        o.order[k] = v
+    return o
+
+
+def _opt_ref(opt):
+    return None if opt is None else _c.byref(opt)
+
+
+def frnn_workspace_bytes(n_total: int, n_events: int = 1, dim: int = 8, k_max: int = 1, opt: FrnnOptions | None = None) -> int:
+    if opt is not None:
+        return int(lib().frnn_workspace_bytes_opt(_c.byref(opt), int(n_total), int(n_events), int(dim), int(k_max)))
     return int(lib().frnn_workspace_bytes(int(n_total), int(n_events), int(dim), int(k_max)))
 
 
@@ -116,10 +163,23 @@ def frnn_set_grid(grid_dims: int = 0, grid_bits: int = 0) -> None:
     _check(lib().frnn_set_grid(int(grid_dims), int(grid_bits)), "frnn_set_grid")
 
 
-def frnn_get_grid(n_total: int, n_events: int = 1) -> tuple[int, int]:
+def frnn_get_grid(n_total: int, n_events: int = 1, dim: int = 8) -> tuple[int, int]:
     d, b = _c.c_int(0), _c.c_int(0)
-    lib().frnn_get_grid(int(n_total), int(n_events), _c.byref(d), _c.byref(b))
+    lib().frnn_get_grid(int(n_total), int(n_events), int(dim), _c.byref(d), _c.byref(b))
     return d.value, b.value
+
+
+def frnn_suggest_grid(points: torch.Tensor, r: float, n_events: int = 1, opt: FrnnOptions | None = None,
+                      stream: torch.cuda.Stream | None = None) -> tuple[FrnnOptions, FrnnGridReport]:
+    """Data-driven choice of (grid_dims, grid_bits, order) for ``points`` (device, n x dim); synchronous."""
+    _require_cuda(points)
+    n, dim = points.shape
+    opt = opt if opt is not None else frnn_options()
+    rep = FrnnGridReport()
+    stream = stream or torch.cuda.current_stream(points.device)
+    _check(lib().frnn_suggest_grid(_ptr(points), n, int(n_events), dim, float(r), _c.byref(opt), _c.byref(rep),
+                                   _c.c_void_p(stream.cuda_stream)), "frnn_suggest_grid")
+    return opt, rep
 
 
 def frnn_set_graph_mode(enabled: bool) -> None:
@@ -198,9 +258,9 @@ class Workspace:
     """Reusable device scratch + output buffers for repeated calls of one shape."""
 
     def __init__(self, n_total: int, n_events: int, k_max: int, edge_capacity: int, device=None, want_row_ptr: bool = False,
-                 dim: int = 8):
+                 dim: int = 8, opt: FrnnOptions | None = None):
         device = device or torch.device("cuda", torch.cuda.current_device())
-        self.bytes = frnn_workspace_bytes(n_total, n_events, dim, k_max)
+        self.bytes = frnn_workspace_bytes(n_total, n_events, dim, k_max, opt)
         self.buf = torch.empty(max(self.bytes, 256), dtype=torch.uint8, device=device)
         self.edge_capacity = int(edge_capacity)
         cap = max(self.edge_capacity, 1)
@@ -221,25 +281,36 @@ def frnn_build_dense_ex(points: torch.Tensor, r: float, k_max: int, edge_capacit
 
 def frnn_build_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int | None = None,
                   ws: Workspace | None = None, stream: torch.cuda.Stream | None = None,
-                  want_row_ptr: bool = False, _entry: str = "frnn_build_ex") -> EdgeList:
-    """Asynchronous single-event build on ``stream`` (default: torch's current stream)."""
+                  want_row_ptr: bool = False, _entry: str = "frnn_build_ex", opt: FrnnOptions | None = None) -> EdgeList:
+    """Asynchronous single-event build on ``stream`` (default: torch's current stream); ``opt``: frnn_build_opt."""
     _require_cuda(points)
     n, dim = points.shape
     if edge_capacity is None:
         edge_capacity = ws.edge_capacity if ws is not None else n * k_max
     if ws is None:
-        ws = Workspace(n, 1, k_max, edge_capacity, points.device, want_row_ptr, dim)
+        ws = Workspace(n, 1, k_max, edge_capacity, points.device, want_row_ptr, dim, opt)
     stream = stream or torch.cuda.current_stream(points.device)
-    st = getattr(lib(), _entry)(_ptr(points), n, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst), _ptr(ws.d2),
-                                int(edge_capacity), _ptr(ws.count), _ptr(ws.status), _ptr(ws.row_ptr),
-                                _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    args = (_ptr(points), n, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst), _ptr(ws.d2),
+            int(edge_capacity), _ptr(ws.count), _ptr(ws.status), _ptr(ws.row_ptr),
+            _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    if opt is not None:
+        assert _entry == "frnn_build_ex"
+        _entry = "frnn_build_opt"
+        st = lib().frnn_build_opt(_c.byref(opt), *args)
+    else:
+        st = getattr(lib(), _entry)(*args)
     _check(st, _entry)
     return EdgeList(ws.src, ws.dst, ws.d2, ws.count, ws.status, ws.row_ptr)
 
 
+def frnn_build_opt(opt: FrnnOptions | None, points: torch.Tensor, r: float, k_max: int, **kw) -> EdgeList:
+    """frnn_build_ex with per-call options."""
+    return frnn_build_ex(points, r, k_max, opt=opt, **kw)
+
+
 def frnn_build_batched(points: torch.Tensor, event_offsets, r: float, k_max: int, edge_capacity: int | None = None,
                        ws: Workspace | None = None, stream: torch.cuda.Stream | None = None,
-                       want_row_ptr: bool = False) -> EdgeList:
+                       want_row_ptr: bool = False, opt: FrnnOptions | None = None) -> EdgeList:
     """Asynchronous batched build: ``event_offsets`` is a host sequence of B+1 ascending row offsets."""
     _require_cuda(points)
     n, dim = points.shape
@@ -248,13 +319,14 @@ def frnn_build_batched(points: torch.Tensor, event_offsets, r: float, k_max: int
     if edge_capacity is None:
         edge_capacity = ws.edge_capacity if ws is not None else n * k_max
     if ws is None:
-        ws = Workspace(n, n_events, k_max, edge_capacity, points.device, want_row_ptr, dim)
+        ws = Workspace(n, n_events, k_max, edge_capacity, points.device, want_row_ptr, dim, opt)
     count = ws.count if ws.count.numel() == n_events + 1 else torch.zeros(n_events + 1, dtype=torch.int64, device=points.device)
     stream = stream or torch.cuda.current_stream(points.device)
     c_offs = (_c.c_int64 * (n_events + 1))(*offs)
-    st = lib().frnn_build_batched(_ptr(points), c_offs, n_events, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst),
-                                  _ptr(ws.d2), int(edge_capacity), _ptr(count), _ptr(ws.status), _ptr(ws.row_ptr),
-                                  _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    args = (_ptr(points), c_offs, n_events, dim, float(r), int(k_max), _ptr(ws.src), _ptr(ws.dst),
+            _ptr(ws.d2), int(edge_capacity), _ptr(count), _ptr(ws.status), _ptr(ws.row_ptr),
+            _ptr(ws.buf), ws.buf.numel(), _c.c_void_p(stream.cuda_stream))
+    st = lib().frnn_build_batched_opt(_c.byref(opt), *args) if opt is not None else lib().frnn_build_batched(*args)
     _check(st, "frnn_build_batched")
     return EdgeList(ws.src, ws.dst, ws.d2, count, ws.status, ws.row_ptr)
 
@@ -331,12 +403,12 @@ def frnn_label_components(n: int, src: torch.Tensor, dst: torch.Tensor, score: t
 class HostPipeline:
     """frnn_host_pipeline_*: a stream of host-resident events with copies and builds overlapped."""
 
-    def __init__(self, n_max: int, k_max: int, edge_capacity: int, depth: int = 3):
+    def __init__(self, n_max: int, k_max: int, edge_capacity: int, depth: int = 3, opt: FrnnOptions | None = None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2202_06929_b200 needs a CUDA device (no CPU fallback)")
         self._h = _c.c_void_p()
-        _check(lib().frnn_host_pipeline_create(int(n_max), 8, int(k_max), int(edge_capacity), int(depth), _c.byref(self._h)),
-               "frnn_host_pipeline_create")
+        _check(lib().frnn_host_pipeline_create_opt(_opt_ref(opt), int(n_max), 8, int(k_max), int(edge_capacity), int(depth),
+                                                   _c.byref(self._h)), "frnn_host_pipeline_create")
 
     def submit(self, points_host: torch.Tensor, r: float, out_src: torch.Tensor, out_dst: torch.Tensor, out_d2: torch.Tensor,
                out_count: torch.Tensor) -> None:

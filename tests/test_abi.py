@@ -55,9 +55,27 @@ def test_host_only_entry_points():
         frnn.frnn_set_grid(0, 0)
     d, b = frnn.frnn_get_grid(120000)
     assert 1 <= d <= 6 and 2 <= b <= 8
+    assert frnn.frnn_get_grid(120000, 1, 2)[0] == 2                    # never more binned coordinates than the rows have
     # the linear cell id (event, cell) must fit 32 bits for any batch size
     d, b = frnn.frnn_get_grid(120000 * 4096, 4096)
     assert d * b + 12 <= 31
+
+
+def test_options_struct_and_sizing():
+    """frnn_options: layout, defaults, validation and workspace sizing (host only)."""
+    o = frnn.frnn_options()
+    assert o.struct_bytes == ctypes.sizeof(frnn.FrnnOptions) == 72
+    assert (o.grid_dims, o.grid_bits, o.order_count, o.launch_mode, o.timeline) == (0, 0, 0, 0, 0)
+    base = frnn.frnn_workspace_bytes(120000, 1, 8, 256)
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, o) == base
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(4, 5)) == base
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(2, 8)) < base          # 65k cells instead of 1M
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(4, 6)) > base
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(order=[3, 1])) == base + (120000 * 4 + 255) // 256 * 256   # slot -> cell array
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(order=[0, 1, 2])) == base   # the default order written out
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(9, 5)) == 0                # invalid options
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(order=[4, 4])) == 0
+    assert frnn.frnn_last_error_string() == ""
 
 
 def test_no_cpu_fallback_without_a_device():
