@@ -182,6 +182,9 @@ int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int
  * capturing the stream, and event-profiled calls always launch one by one.
  */
 int frnn_set_graph_mode(int enabled);
+/* Number of CUDA graphs this process has built and instantiated so far (monotonic).  A stream of calls of one shape on
+ * one workspace must not move it after the first call, whatever n, the buffers and the parameters are. */
+long long frnn_graph_builds(void);
 
 /*
  * The north_star 9-argument form.  Current device, legacy default stream, internally cached

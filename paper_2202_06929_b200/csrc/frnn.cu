@@ -14,6 +14,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
 #include <memory>
 #include <mutex>
 #include <new>
@@ -363,18 +364,23 @@ int launch_plain(const Plan& P, cudaStream_t st) {
 struct ExecEntry {
     void* workspace = nullptr;
     std::vector<const void*> funcs;
+    cudaGraph_t graph = nullptr;  // kept alive: its node handles address the executable's nodes in the update calls
     cudaGraphExec_t exec = nullptr;
     cudaGraphNode_t ms_node = nullptr;
     std::vector<cudaGraphNode_t> knodes;
     Plan held;                    // the parameters the executable currently holds
     uint64_t stamp = 0;
     std::mutex mu;
-    ~ExecEntry() { if (exec) cudaGraphExecDestroy(exec); }
+    ~ExecEntry() {
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
+    }
 };
 std::vector<std::shared_ptr<ExecEntry>> g_execs;
 std::mutex g_exec_mutex;
 uint64_t g_stamp = 0;
 constexpr size_t kMaxExecs = 64;
+std::atomic<long long> g_graph_builds{0};     // frnn_graph_builds(): a stream of calls of one shape must not move it
 
 bool same_shape(const ExecEntry& e, const Plan& P) {
     if (e.funcs.size() != P.nodes.size()) return false;
@@ -407,6 +413,7 @@ cudaMemsetParams memset_params(const Plan& P) {
 // build the executable of entry e from plan P (explicit nodes, a linear chain)
 int build_exec(ExecEntry& e, const Plan& P) {
     if (e.exec) { cudaGraphExecDestroy(e.exec); e.exec = nullptr; }
+    if (e.graph) { cudaGraphDestroy(e.graph); e.graph = nullptr; }
     e.knodes.clear();
     cudaGraph_t graph = nullptr;
     CK(cudaGraphCreate(&graph, 0));
@@ -423,8 +430,9 @@ int build_exec(ExecEntry& e, const Plan& P) {
         prev = node;
     }
     if (err == cudaSuccess) err = cudaGraphInstantiate(&e.exec, graph, 0);
-    cudaGraphDestroy(graph);
-    if (err != cudaSuccess) { e.exec = nullptr; return cuda_fail(err, "building the CUDA graph"); }
+    if (err != cudaSuccess) { cudaGraphDestroy(graph); e.exec = nullptr; return cuda_fail(err, "building the CUDA graph"); }
+    e.graph = graph;
+    g_graph_builds.fetch_add(1, std::memory_order_relaxed);
     e.held = P;                                                // (e.funcs, the identity of the entry, was set at creation)
     return FRNN_OK;
 }
@@ -478,7 +486,7 @@ int launch_graph(const Plan& P, void* workspace, cudaStream_t st) {
     std::lock_guard<std::mutex> lock(e->mu);
     int rc = FRNN_OK;
     if (!e->exec) rc = build_exec(*e, P);
-    else if ((rc = update_exec(*e, P)) != FRNN_OK) rc = build_exec(*e, P);     // an update the driver refuses: start over
+    else if ((rc = update_exec(*e, P)) != FRNN_OK) rc = build_exec(*e, P);     // an update the driver refuses: start over (counted, see frnn_graph_builds)
     if (rc != FRNN_OK) return rc;
     CK(cudaGraphLaunch(e->exec, st));
     t_launches = static_cast<int>(P.nodes.size()) + 1;
@@ -1112,6 +1120,8 @@ void frnn_host_pipeline_destroy(frnn_host_pipeline* p) {
 }
 
 int frnn_last_launch_count(void) { return t_launches; }
+
+long long frnn_graph_builds(void) { return g_graph_builds.load(std::memory_order_relaxed); }
 
 int frnn_set_profiling(int enabled) {
     {

@@ -91,6 +91,24 @@ def one_cluster(n: int, sigma: float, seed: int) -> np.ndarray:
     return np.ascontiguousarray(rng.normal(0.0, sigma, (n, DIM)).astype(np.float32))
 
 
+def dense_tracks(n: int, hits_per_track: float, sigma: float, seed: int) -> np.ndarray:
+    """A dense event: ``n`` points in tracks of Poisson(hits_per_track) hits (min 3) around U[-1,1]^8 centres with
+    N(0, sigma^2) spread, rows permuted.  With hits_per_track = 200, sigma = 0.02 and r = 0.1 the mean degree is about
+    170: the regime BASELINE.json's config-4 parenthetical "(mean degree ~200)" describes and its recipe does not reach
+    (R14); used for the K-binding bench leg and parity tests."""
+    rng = np.random.default_rng(seed)
+    t = max(int(round(n / hits_per_track)), 1)
+    counts = np.maximum(rng.poisson(hits_per_track, t), 3).astype(np.int64)
+    centres = rng.uniform(-1.0, 1.0, (t, DIM))
+    tid = np.repeat(np.arange(t), counts)
+    if len(tid) >= n:
+        tid = tid[:n]
+    else:
+        tid = np.concatenate([tid, rng.integers(0, t, n - len(tid))])
+    x = (centres[tid] + rng.normal(0.0, sigma, (n, DIM))).astype(np.float32)
+    return np.ascontiguousarray(x[rng.permutation(n)])
+
+
 def lattice(length: int, dim: int, h: float) -> np.ndarray:
     """Cubic lattice of ``length**dim`` points, spacing ``h``, centred on the origin.
 

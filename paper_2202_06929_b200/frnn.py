@@ -69,6 +69,7 @@ _SIGNATURES = {
                                    _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64, _c.POINTER(_c.c_int64)]),
     "frnn_last_launch_count": (_c.c_int, []),
     "frnn_set_graph_mode": (_c.c_int, [_c.c_int]),
+    "frnn_graph_builds": (_c.c_longlong, []),
     "frnn_set_profiling": (_c.c_int, [_c.c_int]),
     "frnn_get_profile": (_c.c_int, [_c.POINTER(_c.c_float), _c.c_int]),
     "frnn_phase_name": (_c.c_char_p, [_c.c_int]),
@@ -184,6 +185,10 @@ def frnn_suggest_grid(points: torch.Tensor, r: float, n_events: int = 1, opt: Fr
 
 def frnn_set_graph_mode(enabled: bool) -> None:
     _check(lib().frnn_set_graph_mode(int(bool(enabled))), "frnn_set_graph_mode")
+
+
+def frnn_graph_builds() -> int:
+    return int(lib().frnn_graph_builds())
 
 
 def frnn_last_launch_count() -> int:

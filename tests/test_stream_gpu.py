@@ -74,10 +74,12 @@ def test_more_than_128_distinct_sizes_through_one_workspace(F):
         o.buf = ws.buf
     results = []
     launch_counts = set()
+    builds = []
     for i, n in enumerate(sizes):
         o = outs[i % 3]
         res = F.frnn_build_ex(dev_in[i % 5][:n], cfg.r, cfg.k_max, ws=o, stream=stream)
         launch_counts.add(F.frnn_last_launch_count())
+        builds.append(F.frnn_graph_builds())
         if i % 3 == 2 or i == len(sizes) - 1:                                  # the three output sets are full: check them
             stream.synchronize()
             for j in range(i - (i % 3), i + 1):
@@ -86,6 +88,7 @@ def test_more_than_128_distinct_sizes_through_one_workspace(F):
                 assert int(r_.status.item()) == 0
                 results.append((j, r_.src[:e].cpu().numpy(), r_.dst[:e].cpu().numpy(), r_.d2[:e].cpu().numpy()))
     assert launch_counts == {6}, launch_counts                                 # memset + 5 kernels, every time
+    assert builds[-1] == builds[0], "the graph was rebuilt although only n and the buffers changed"
     assert len(results) == 150
     for j, s, d, q in results:
         n = sizes[j]
@@ -102,11 +105,14 @@ def test_sizes_across_grid_classes_and_back(F):
     need3 = F.frnn_workspace_bytes(16000, 1, 8, cfg.k_max)
     assert need3 <= ws.buf.numel()
     st = torch.cuda.Stream()
+    b0 = F.frnn_graph_builds()
     for n in (20000, 5000, 17000, 16383, 16384, 1, 2, 300, 19999):
         res = F.frnn_build_ex(pts[:n], cfg.r, cfg.k_max, ws=ws, stream=st)
         st.synchronize()
         res.check()
         assert_same(host_result(res), oracle.frnn(x[:n], cfg.r, cfg.k_max, oracle.CELLS), cfg.r, f"n={n}")
+    assert F.frnn_graph_builds() - b0 <= 2                                     # one graph per grid class, reused (none if an earlier
+                                                                               # workspace at this address left them behind)
 
 
 def test_batched_calls_with_changing_offsets_replay_one_graph(F):
@@ -116,6 +122,7 @@ def test_batched_calls_with_changing_offsets_replay_one_graph(F):
     total_max = 6 * cfg.n
     ws = F.Workspace(total_max, 6, 5, total_max * 5)
     rng = np.random.default_rng(3)
+    b0 = None
     for trial in range(5):
         sizes = rng.integers(0, cfg.n, 6)
         x = np.ascontiguousarray(np.concatenate([e[:m] for e, m in zip(evs, sizes)]))
@@ -131,6 +138,8 @@ def test_batched_calls_with_changing_offsets_replay_one_graph(F):
         assert np.array_equal(res.count.cpu().numpy(), eoffs)
         s, d, q = (t.cpu().numpy() for t in res.trimmed())
         assert np.array_equal(s, exp.src) and np.array_equal(d, exp.dst) and np.array_equal(H.bits(q), H.bits(exp.d2))
+        b0 = F.frnn_graph_builds() if b0 is None else b0
+    assert F.frnn_graph_builds() == b0                                         # the offsets changed, the graph did not
 
 
 def test_plain_launch_mode_and_graph_mode_agree(F):
