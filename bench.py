@@ -529,14 +529,15 @@ def main() -> None:
         radius_sweep = []
         p_dev = pts[0]
         for rr in (0.02, 0.05, 0.1, 0.2):
-            opt, rep = F.frnn_suggest_grid(p_dev, rr)
+            opt, rep = F.frnn_suggest_grid(p_dev, rr, measure=True)
             ecap = n * (64 if rr > 0.15 else EDGE_CAP_PER_ROW)
             ms_s, e_s, _, _ = time_single(host_events[0], rr, k_max, reps, opt=opt, cap_edges=ecap)
             ms_d, e_d, _, _ = time_single(host_events[0], rr, k_max, reps, cap_edges=ecap)
             assert e_s == e_d
             row = {"r": rr, "edges": e_s, "suggested": {"grid_dims": opt.grid_dims, "grid_bits": opt.grid_bits, "reordered": bool(rep.reordered),
                                                         "ms_per_event": ms_s, "predicted_candidates_per_query": rep.predicted_candidates,
-                                                        "predicted_us": rep.predicted_us},
+                                                        "predicted_us": rep.predicted_us, "measured_us_capacity0": rep.measured_us,
+                                                        "shortlist": rep.tried()},
                    "default": {"grid": list(F.frnn_get_grid(n, 1, 8)), "ms_per_event": ms_d},
                    "extent_cells": rep.extent_cells[0]}
             if not rep.reordered:

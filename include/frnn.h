@@ -131,25 +131,35 @@ void frnn_get_grid(int64_t n_total, int n_events, int dim, int* grid_dims, int* 
  * torus; the expected candidates per query of a grid are n * product of s over its binned coordinates, the survivors
  * of the key filter that times the product of s(64 cells) over the keyed ones.  It then picks the (grid_dims,
  * grid_bits) -- and, only when that is predicted to gain more than 10 %, an order of the coordinates -- that minimise
- * a cost model of the path (table entries to zero and scan; per query: neighbour rows, keys, survivors; constants in
- * DESIGN.md section 7), over grids whose table stays within 32 cells per point of an event, and writes the choice
- * into *opt (which must have been initialised; launch_mode and timeline are left alone).  *report (optional)
- * receives what it saw and what it predicts.  The statistics of an embedding belong to the trained model more than
- * to the event: choose once per model and radius, reuse the options -- the per-event path stays reduction-free.
- * SYNCHRONOUS (one small kernel, a stream synchronise).  Never changes any result.
+ * a cost model of the path (fixed latency; table entries to zero and scan; per query: neighbour rows, keys, survivors;
+ * constants in DESIGN.md section 7), over grids whose table stays within 32 cells per point of an event.
+ *   measure == 0: the model's best is taken as it is (one small kernel, a stream synchronise).
+ *   measure != 0: the model only makes a SHORTLIST (at most FRNN_GRID_REPORT_TRIES grids within 2.5x of its best); each
+ *                 is then run for real on the first event of `points` (edge capacity 0: everything but the output
+ *                 stores; plain launches; 1 warm-up + 3 timed calls, CUDA events on cuda_stream) and the fastest wins.
+ *                 Allocates and frees its own scratch (cudaMalloc); a few milliseconds: a set-up call.
+ * The choice is written into *opt (which must have been initialised; launch_mode and timeline are left alone); an
+ * order of the coordinates other than the default is chosen only for a predicted gain of more than 10 %.  *report
+ * (optional) receives what was seen, predicted and measured.  The statistics of an embedding belong to the trained
+ * model more than to the event: choose once per model and radius, reuse the options -- the per-event path stays
+ * reduction-free.  SYNCHRONOUS.  Never changes any result.
  */
+#define FRNN_GRID_REPORT_TRIES 12
 typedef struct frnn_grid_report {
-    int32_t grid_dims, grid_bits, reordered;
+    int32_t grid_dims, grid_bits, reordered, n_tried;
     int64_t sampled;                 /* rows looked at */
     float predicted_candidates;      /* per query, both directions */
     float predicted_survivors;       /* candidates that pass the key filter, per query */
     float predicted_us;              /* the cost model's figure for one call */
+    float measured_us;               /* measure != 0: device time of one call on the chosen grid (capacity 0) */
     float extent_cells[16];          /* (max - min) / cell side per coordinate */
     float pair_probability[16];      /* s at the chosen grid_bits per coordinate */
     float key_probability[16];       /* s at the key filter's 64 cells per coordinate */
+    int32_t tried_dims[FRNN_GRID_REPORT_TRIES], tried_bits[FRNN_GRID_REPORT_TRIES], tried_reordered[FRNN_GRID_REPORT_TRIES];
+    float tried_predicted_us[FRNN_GRID_REPORT_TRIES], tried_measured_us[FRNN_GRID_REPORT_TRIES];   /* the shortlist */
 } frnn_grid_report;
-int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, float r, frnn_options* opt /* HOST, in/out */,
-                      frnn_grid_report* report /* HOST, optional */, void* cuda_stream);
+int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, float r, int measure,
+                      frnn_options* opt /* HOST, in/out */, frnn_grid_report* report /* HOST, optional */, void* cuda_stream);
 
 /*
  * Which coordinates the grid bins and which the key filter tests (PAPER.md:69 says only that the

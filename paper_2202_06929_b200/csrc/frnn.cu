@@ -18,6 +18,7 @@
 #include <memory>
 #include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "../../include/frnn.h"
@@ -691,12 +692,16 @@ double pair_probability(const unsigned int* h256, int bits, double total) {
     return acc;
 }
 
-// Cost model of one event on the grid (g, bits) in microseconds of device time, fitted to the sweeps recorded in
-// DESIGN.md section 7 (B200): table entries pay for the memset and the scan, every query pays per neighbour row
-// (two table reads + bookkeeping: the 3^(g-1) term of PAPER.md:69), per candidate key tested and per survivor row
-// evaluated.  Only the ranking of the alternatives matters; the result never depends on the choice.
+// Cost model of one call on the grid (g, bits) in microseconds of device time, fitted to the sweeps recorded in
+// DESIGN.md section 7 (B200): a fixed part (launch and dependency latency of the six graph nodes), the table entries to
+// zero and scan, per query the neighbour rows (the 3^(g-1) term of PAPER.md:69: two table reads and bookkeeping per row,
+// with a latency term of its own for g >= 4 because a thread walks its rows one sub-batch after the other) and the
+// candidate keys tested, dearer beyond the first four of a run (they take the merged leftover loop).  The model only
+// has to RANK the alternatives well enough for the true best to make the shortlist that is then measured.
 struct GridCost { double us, cand, surv; };
 GridCost grid_cost(const double s[kDimMax][9], const unsigned char* order, int dim, int g, int bits, double n_event, int n_events) {
+    static const double kRowLatency[7] = {0, 0, 0, 0.5, 4.7, 46.0, 90.0};          // us, whatever n is
+    static const double kRowsPer100k[7] = {0, 0, 0, 1.2, 13.9, 37.4, 110.0};       // us per 100,000 queries
     double cand = n_event;
     for (int d = 0; d < g; ++d) cand *= order[d] < dim ? s[order[d]][bits] : 1.0;
     double surv = cand;
@@ -706,12 +711,15 @@ GridCost grid_cost(const double s[kDimMax][9], const unsigned char* order, int d
     for (int d = 0; d + 1 < g; ++d) runs *= 3.0;
     const double entries = static_cast<double>(n_events) * pow(2.0, g * bits) * (1.0 + pow(2.0, -bits));
     const double n_all = n_event * n_events;
+    const double beyond = fmax(0.0, cand - 4.0 * runs);                            // candidates past the first four of their run
     GridCost c;
     c.cand = cand;
     c.surv = surv;
-    c.us = 2.0e-6 * entries + n_all * (4.9e-6 * runs * (g >= 5 ? 2.0 : 1.0) + 0.53e-6 * cand + 6.0e-6 * surv);
+    c.us = 23.0 + kRowLatency[g] + 2.0e-6 * entries + n_all * (1e-5 * kRowsPer100k[g] + 0.35e-6 * cand + 1.2e-6 * beyond + 6.0e-6 * surv);
     return c;
 }
+
+struct GridTry { int g, bits, order; GridCost c; float measured_us; };
 
 }  // namespace
 
@@ -790,61 +798,133 @@ int frnn_suggest_bin_order(const float* points, int64_t n, int dim, float r, int
     return FRNN_OK;
 }
 
-int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, float r, frnn_options* opt, frnn_grid_report* report,
-                      void* cuda_stream) {
+int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, float r, int measure, frnn_options* opt,
+                      frnn_grid_report* report, void* cuda_stream) {
     if (!points || !opt || n < 1 || n_events < 1 || !(r >= 0.0f) || !isfinite(r)) return FRNN_ERR_INVALID_ARG;
     if (dim < 1 || dim > kDimMax) return FRNN_ERR_UNSUPPORTED;
     if (opt->struct_bytes < sizeof(frnn_options)) return FRNN_ERR_INVALID_ARG;
+    if (dim == kDim && reinterpret_cast<uintptr_t>(points) % 32) return FRNN_ERR_INVALID_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     SuggestOut so;
-    const int rc = run_suggest(points, n, dim, r, static_cast<cudaStream_t>(cuda_stream), &so);
+    int rc = run_suggest(points, n, dim, r, st, &so);
     if (rc != FRNN_OK) return rc;
     const double tot = so.sampled ? static_cast<double>(so.sampled) : 1.0;
     double s[kDimMax][9];
     for (int d = 0; d < kDimMax; ++d)
         for (int b = 0; b <= 8; ++b) s[d][b] = (d < dim && b >= 2) ? pair_probability(so.hist[d], b, tot) : 1.0;
     // two candidate orders: the default one and the coordinates ranked by how much they prune (at the key's 64 cells)
-    unsigned char ident[8] = {0, 1, 2, 3, 4, 5, 6, 7}, ranked[8];
+    unsigned char orders[2][8] = {{0, 1, 2, 3, 4, 5, 6, 7}, {0, 1, 2, 3, 4, 5, 6, 7}};
     {
         int idx[kDimMax];
         for (int d = 0; d < kDimMax; ++d) idx[d] = d;
         for (int a = 1; a < kDimMax; ++a)
             for (int b = a; b > 0 && s[idx[b]][6] < s[idx[b - 1]][6]; --b) { const int t = idx[b]; idx[b] = idx[b - 1]; idx[b - 1] = t; }
-        for (int k = 0; k < 8; ++k) ranked[k] = static_cast<unsigned char>(idx[k]);
+        for (int k = 0; k < 8; ++k) orders[1][k] = static_cast<unsigned char>(idx[k]);
     }
+    const int64_t n_first = n / n_events > 0 ? n / n_events : n;                  // rows of the sample event that is measured
     const double n_event = static_cast<double>(n) / n_events;
     int ev_bits = 0;
     while ((1ll << ev_bits) < n_events) ++ev_bits;
     // table budget: 32 cells per point of an event (a finer table costs more to zero and scan than it saves), 2^26 in all
     const double budget = fmin(fmax(65536.0, 32.0 * n_event), 67108864.0 / n_events);
-    struct Best { GridCost c; int g, bits; bool ok; } best[2] = {{{0, 0, 0}, 0, 0, false}, {{0, 0, 0}, 0, 0, false}};
-    for (int which = 0; which < 2; ++which) {
-        const unsigned char* ord = which ? ranked : ident;
-        for (int g = 1; g <= 6 && g <= dim; ++g)
-            for (int bits = 2; bits <= 8; ++bits) {
-                if (g * bits + ev_bits > 30 || pow(2.0, g * bits) > budget) continue;
-                const GridCost c = grid_cost(s, ord, dim, g, bits, n_event, n_events);
-                if (!best[which].ok || c.us < best[which].c.us) best[which] = Best{c, g, bits, true};
+    std::vector<GridTry> all;
+    const bool same_order = memcmp(orders[0], orders[1], 8) == 0;
+    for (int g = 1; g <= 6 && g <= dim; ++g)
+        for (int bits = 2; bits <= 8; ++bits) {
+            if (g * bits + ev_bits > 30 || pow(2.0, g * bits) > budget) continue;
+            GridTry t{g, bits, 0, grid_cost(s, orders[0], dim, g, bits, n_event, n_events), 0.0f};
+            if (!same_order) {                     // reorder only for a clear predicted gain: the default order is the fast path
+                const GridCost c1 = grid_cost(s, orders[1], dim, g, bits, n_event, n_events);
+                if (c1.us < 0.9 * t.c.us) { t.order = 1; t.c = c1; }
             }
-    }
-    if (!best[0].ok) return FRNN_ERR_UNSUPPORTED;
-    const int pick = (best[1].ok && best[1].c.us < 0.9 * best[0].c.us) ? 1 : 0;     // reorder only for a clear gain: the default order is the fast path
-    opt->grid_dims = best[pick].g;
-    opt->grid_bits = best[pick].bits;
-    opt->order_count = pick ? 8 : 0;
-    for (int k = 0; k < 8; ++k) opt->order[k] = pick ? ranked[k] : k;
-    if (report) {
+            all.push_back(t);
+        }
+    if (all.empty()) return FRNN_ERR_UNSUPPORTED;
+    for (size_t a = 1; a < all.size(); ++a)                                        // by predicted cost
+        for (size_t b = a; b > 0 && all[b].c.us < all[b - 1].c.us; --b) std::swap(all[b], all[b - 1]);
+    size_t pick = 0, n_tried = 0;
+    if (measure) {
+        // the shortlist, run for real on the first event of the sample: capacity 0 (no output is written, everything else
+        // runs), plain launches (no graph is left behind), 1 warm-up + 3 timed calls each, CUDA events on the stream
+        std::vector<size_t> shortlist;
+        for (size_t k = 0; k < all.size() && shortlist.size() < static_cast<size_t>(FRNN_GRID_REPORT_TRIES); ++k) {
+            if (all[k].c.us > 2.5 * all[0].c.us) break;
+            shortlist.push_back(k);
+        }
+        size_t ws_bytes = 0;
+        std::vector<Opts> so_opts(shortlist.size());
+        for (size_t k = 0; k < shortlist.size(); ++k) {
+            Opts& o = so_opts[k];
+            o.grid_dims = all[shortlist[k]].g;
+            o.grid_bits = all[shortlist[k]].bits;
+            int ord[8];
+            for (int q = 0; q < 8; ++q) ord[q] = orders[all[shortlist[k]].order][q];
+            make_order(ord, all[shortlist[k]].order ? 8 : 0, &o.order);
+            o.use_graph = false;
+            const size_t b = workspace_bytes_for(o, n_first, 1, dim, 1 << 20);
+            if (b > ws_bytes) ws_bytes = b;
+        }
+        void* ws = nullptr;
+        int64_t* d_misc = nullptr;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        cudaError_t ce = cudaMalloc(&ws, ws_bytes);
+        if (ce == cudaSuccess) ce = cudaMalloc(reinterpret_cast<void**>(&d_misc), 64);
+        if (ce == cudaSuccess) ce = cudaEventCreate(&e0);
+        if (ce == cudaSuccess) ce = cudaEventCreate(&e1);
+        rc = ce == cudaSuccess ? FRNN_OK : cuda_fail(ce, "frnn_suggest_grid: scratch for the measured shortlist");
+        float best_us = 0.0f;
+        for (size_t k = 0; rc == FRNN_OK && k < shortlist.size(); ++k) {
+            for (int rep = 0; rep < 4 && rc == FRNN_OK; ++rep) {
+                if (rep == 1) cudaEventRecord(e0, st);
+                rc = build_single(so_opts[k], false, points, n_first, dim, r, 1 << 20, nullptr, nullptr, nullptr, 0, d_misc,
+                                  reinterpret_cast<int32_t*>(d_misc + 1), nullptr, ws, ws_bytes, st);
+            }
+            if (rc != FRNN_OK) break;
+            cudaEventRecord(e1, st);
+            ce = cudaEventSynchronize(e1);
+            float ms = 0.0f;
+            if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+            if (ce != cudaSuccess) { rc = cuda_fail(ce, "frnn_suggest_grid: timing"); break; }
+            all[shortlist[k]].measured_us = 1e3f * ms / 3.0f;
+            if (k == 0 || all[shortlist[k]].measured_us < best_us) { best_us = all[shortlist[k]].measured_us; pick = shortlist[k]; }
+        }
+        if (e0) cudaEventDestroy(e0);
+        if (e1) cudaEventDestroy(e1);
+        if (d_misc) cudaFree(d_misc);
+        if (ws) cudaFree(ws);
+        if (rc != FRNN_OK) return rc;
+        n_tried = shortlist.size();
+        if (report) {
+            memset(report, 0, sizeof(*report));
+            for (size_t k = 0; k < shortlist.size(); ++k) {
+                const GridTry& t = all[shortlist[k]];
+                report->tried_dims[k] = t.g; report->tried_bits[k] = t.bits; report->tried_reordered[k] = t.order;
+                report->tried_predicted_us[k] = static_cast<float>(t.c.us);
+                report->tried_measured_us[k] = t.measured_us;
+            }
+        }
+    } else if (report) {
         memset(report, 0, sizeof(*report));
-        report->grid_dims = best[pick].g;
-        report->grid_bits = best[pick].bits;
-        report->reordered = pick;
+    }
+    const GridTry& best = all[pick];
+    opt->grid_dims = best.g;
+    opt->grid_bits = best.bits;
+    opt->order_count = best.order ? 8 : 0;
+    for (int k = 0; k < 8; ++k) opt->order[k] = best.order ? orders[1][k] : k;
+    if (report) {
+        report->grid_dims = best.g;
+        report->grid_bits = best.bits;
+        report->reordered = best.order;
+        report->n_tried = static_cast<int32_t>(n_tried);
         report->sampled = static_cast<int64_t>(so.sampled);
-        report->predicted_candidates = static_cast<float>(best[pick].c.cand);
-        report->predicted_survivors = static_cast<float>(best[pick].c.surv);
-        report->predicted_us = static_cast<float>(best[pick].c.us);
+        report->predicted_candidates = static_cast<float>(best.c.cand);
+        report->predicted_survivors = static_cast<float>(best.c.surv);
+        report->predicted_us = static_cast<float>(best.c.us);
+        report->measured_us = best.measured_us;
         const float side = fmaxf(r * kCellSlack, 1e-30f);
         for (int d = 0; d < kDimMax; ++d) {
             report->extent_cells[d] = d < dim ? (so.hi[d] - so.lo[d]) / side : 0.0f;
-            report->pair_probability[d] = d < dim ? static_cast<float>(s[d][best[pick].bits]) : 1.0f;
+            report->pair_probability[d] = d < dim ? static_cast<float>(s[d][best.bits]) : 1.0f;
             report->key_probability[d] = d < dim ? static_cast<float>(s[d][6]) : 1.0f;
         }
     }

@@ -176,6 +176,12 @@ __device__ __forceinline__ void stamp_end(unsigned long long* stamps, int phase)
     if (stamps && threadIdx.x == 0) atomicMax(&stamps[2 * phase + 1], global_ns());
 }
 
+// The same for kernels whose threads finish at very different times (search, the warp loops of emit): the LAST thread of
+// the block to arrive stamps the end (a shared-memory counter; only touched when the timeline is being recorded).
+__device__ __forceinline__ void stamp_end_last(unsigned long long* stamps, int phase, unsigned int* s_done) {
+    if (stamps && atomicAdd(s_done, 1u) == blockDim.x - 1u) atomicMax(&stamps[2 * phase + 1], global_ns());
+}
+
 // dims 8..15 of a pair: the chain simply goes on (R3: one fp32 chain over d = 0..dim-1 in index order)
 __device__ __forceinline__ float d2_continue(float acc, const float4& qc, const float4& qd, const float4& cc, const float4& cd) {
     float t;
@@ -564,10 +570,15 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     constexpr int kWide = 4;                              // survivors evaluated together (rows in flight per thread)
     __shared__ uint32_t s_queue[kQueue][kSearchThreads];
     __shared__ __align__(8) uint2 s_left[kLeft][kSearchThreads];      // leftover runs (first slot, length), one column per thread
+    __shared__ unsigned int s_done;                                   // timeline only: threads of the block that have finished
     stamp_begin(a.stamps, 3);
     const int tid = threadIdx.x;
+    if (a.stamps) {                                                   // (kernel argument: uniform)
+        if (tid == 0) s_done = 0u;
+        __syncthreads();
+    }
     const int64_t s64 = static_cast<int64_t>(blockIdx.x) * kSearchThreads + tid;
-    if (s64 >= a.n_total) { stamp_end(a.stamps, 3); return; }      // no block-wide barrier below
+    if (s64 >= a.n_total) { stamp_end_last(a.stamps, 3, &s_done); return; }      // no block-wide barrier below
     const uint32_t s = static_cast<uint32_t>(s64);
     float4 qa, qb;
     load_row_nc(a.spts + 2 * s64, qa, qb);
@@ -803,7 +814,7 @@ __global__ void __launch_bounds__(kSearchThreads, FRNN_SEARCH_MIN_BLOCKS) search
     drain(true);
     // per-tile degree totals: emit_kernel turns them into its global offsets without any inter-block wait
     if (own_deg) atomicAdd(&my_tile_deg[my_row / kEmitThreads], static_cast<unsigned long long>(own_deg));
-    stamp_end(a.stamps, 3);
+    stamp_end_last(a.stamps, 3, &s_done);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -930,13 +941,16 @@ __global__ void __launch_bounds__(kPrefixThreads) tile_prefix_kernel(PrefixArgs 
 //                                under (d2, j) among the row's hits decides whether it is kept (rank < K); a second
 //                                sweep places the kept hits by dst among the kept
 //   big     c > kSlot            the slot buffer overflowed: the row is recomputed by a whole warp, ONE pass over
-//                                its neighbourhood collecting the in-radius hits as 64-bit keys (d2 bits, j) into
-//                                the warp's staging buffer in shared memory (kStage entries); if c > K a bitonic
-//                                sort of the keys keeps the K smallest (north_star (3): warp-level bitonic top-K
-//                                on (d2, index) with index tie-break), a second sort orders the kept by dst
-//   huge    c > kStage           beyond the staging capacity: threshold by storage-free bisection on the bit
-//                                pattern of d2 and then on j among ties (one neighbourhood pass per step), hits
-//                                written unsorted and ordered in place by a bitonic network in global memory
+//                                its neighbourhood; in-radius hits below the current threshold go as 64-bit keys
+//                                (d2 bits, j) into the warp's staging buffer in shared memory (kStage entries).
+//                                When the buffer fills up (c > kStage) and at the end (c > K) it is pruned to the K
+//                                smallest keys by warp_select_keys -- north_star (3): warp-level top-K on (d2, index)
+//                                with index tie-break -- and the K-th key becomes the threshold: a streaming top-K
+//                                that serves any count as long as K <= kStage / 2.  A bitonic network then orders
+//                                the kept keys by dst.
+//   huge    c > kStage and K > kStage / 2: threshold by storage-free bisection on the bit pattern of d2 and then on
+//                                j among ties (one neighbourhood pass per step), hits written unsorted and ordered
+//                                in place by a bitonic network in global memory
 // ------------------------------------------------------------------------------------------------
 constexpr int kStage = 512;            // staging entries per warp for recomputed rows (K <= 512: 16 keys per lane)
 
@@ -987,6 +1001,57 @@ __device__ __forceinline__ void warp_sort_keys(unsigned long long* k, int p2, in
             __syncwarp();
         }
     }
+}
+
+// Warp top-K on staged keys (north_star (3): per-query K-cap selection on (d2, index) with index tie-break): the k
+// smallest of the n distinct 64-bit keys key[0..n) (d2 bits << 32 | j, d2 bits <= hi_max) are moved to key[0..k), in no
+// particular order, and the k-th smallest key is returned.  Bisection on the bit pattern of d2 (every step counts, with
+// one pass over the staged keys and a warp reduction, how many lie at or below the probe), then -- only if several keys
+// share the k-th d2 and not all of them are wanted -- on j among those; then a stable in-place compaction.  n <= kStage,
+// 1 <= k < n.  All lanes must call it; the caller has made the staged keys visible (__syncwarp).
+__device__ __forceinline__ unsigned long long warp_select_keys(unsigned long long* key, uint32_t n, uint32_t k, uint32_t hi_max,
+                                                               int lane, uint32_t lt_mask) {
+    const uint32_t* w = reinterpret_cast<const uint32_t*>(key);       // w[2t] = j, w[2t+1] = d2 bits (little endian)
+    uint32_t lo = 0, hi = hi_max;
+    while (lo < hi) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        uint32_t c = 0;
+        for (uint32_t t = lane; t < n; t += 32) c += w[2 * t + 1] <= mid;
+        c = __reduce_add_sync(kFull, c);
+        if (c >= k) hi = mid; else lo = mid + 1;
+    }
+    const uint32_t dk = lo;                                           // the k-th smallest d2
+    uint32_t c_lt = 0, c_eq = 0;
+    for (uint32_t t = lane; t < n; t += 32) { const uint32_t d = w[2 * t + 1]; c_lt += d < dk; c_eq += d == dk; }
+    c_lt = __reduce_add_sync(kFull, c_lt);
+    c_eq = __reduce_add_sync(kFull, c_eq);
+    const uint32_t need = k - c_lt;                                   // how many of the keys with d2 == dk are wanted (>= 1)
+    uint32_t jk = 0x7fffffffu;
+    if (need < c_eq) {                                                // ties at the k-th d2: the smallest indices win
+        uint32_t jlo = 0, jhi = 0x7fffffffu;
+        while (jlo < jhi) {
+            const uint32_t mid = jlo + ((jhi - jlo) >> 1);
+            uint32_t c = 0;
+            for (uint32_t t = lane; t < n; t += 32) c += (w[2 * t + 1] == dk) && (w[2 * t] <= mid);
+            c = __reduce_add_sync(kFull, c);
+            if (c >= need) jhi = mid; else jlo = mid + 1;
+        }
+        jk = jlo;
+    }
+    const unsigned long long thr = (static_cast<unsigned long long>(dk) << 32) | jk;
+    // compaction, 32 keys at a time in index order: everything a chunk writes lies at or before the chunk itself
+    uint32_t out = 0;
+    for (uint32_t t0 = 0; t0 < n; t0 += 32) {
+        const uint32_t t = t0 + lane;
+        const unsigned long long v = t < n ? key[t] : ~0ull;
+        const bool keep = v <= thr;
+        const uint32_t m = __ballot_sync(kFull, keep);
+        __syncwarp();
+        if (keep) key[out + __popc(m & lt_mask)] = v;
+        out += __popc(m);
+        __syncwarp();
+    }
+    return thr;
 }
 
 struct EmitArgs {
@@ -1066,30 +1131,37 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
     const int32_t src = static_cast<int32_t>(row - row_ev);
     const uint32_t kept = row_cnt < a.k_max ? row_cnt : a.k_max;
 
-    if (row_cnt <= static_cast<uint32_t>(kStage)) {
-        // ---- ONE pass: every in-radius hit becomes a key (d2 bits << 32 | j) in the staging buffer.  d2 >= +0 always
-        // (the chain starts at +0 and adds squares), so bit patterns order like values and the key order IS (d2, j).
-        uint32_t off = 0;
+    if (row_cnt <= static_cast<uint32_t>(kStage) || a.k_max <= static_cast<uint32_t>(kStage / 2)) {
+        // ---- ONE pass: an in-radius hit becomes a key (d2 bits << 32 | j) in the staging buffer if it is below the current
+        // threshold (initially none).  d2 >= +0 always (the chain starts at +0 and adds squares), so bit patterns order
+        // like values and the key order IS (d2, j); keys are distinct (j is).  When the buffer is about to fill up, it is
+        // pruned to the K smallest keys (warp_select_keys) and the K-th becomes the threshold: a streaming top-K, any count.
+        uint32_t fill = 0;
+        unsigned long long thr = ~0ull;
         visit([&](bool in, int32_t cj, float d2) {
-            const uint32_t m = __ballot_sync(kFull, in);
-            if (in) {
-                const uint32_t at = off + __popc(m & lt_mask);
-                if (at < static_cast<uint32_t>(kStage))
-                    stage[at] = (static_cast<unsigned long long>(__float_as_uint(d2)) << 32) | static_cast<uint32_t>(cj);
+            const unsigned long long key = (static_cast<unsigned long long>(__float_as_uint(d2)) << 32) | static_cast<uint32_t>(cj);
+            const bool take = in && key < thr;
+            const uint32_t m = __ballot_sync(kFull, take);
+            if (take) {
+                const uint32_t at = fill + __popc(m & lt_mask);
+                if (at < static_cast<uint32_t>(kStage)) stage[at] = key;
             }
-            off += __popc(m);
+            fill += __popc(m);
+            if (fill > static_cast<uint32_t>(kStage - 32) && fill > a.k_max) {       // (K <= kStage / 2 here, or the row would fit)
+                __syncwarp();
+                thr = warp_select_keys(stage, fill < static_cast<uint32_t>(kStage) ? fill : static_cast<uint32_t>(kStage), a.k_max,
+                                       __float_as_uint(a.r2), lane, lt_mask);
+                fill = a.k_max;
+            }
         });
-        uint32_t len = off < static_cast<uint32_t>(kStage) ? off : static_cast<uint32_t>(kStage);    // == row_cnt
         __syncwarp();
-        if (len > a.k_max) {                              // S8: the K smallest keys
-            int p2 = 2;
-            while (static_cast<uint32_t>(p2) < len) p2 <<= 1;
-            for (int t = static_cast<int>(len) + lane; t < p2; t += 32) stage[t] = ~0ull;
-            __syncwarp();
-            warp_sort_keys(stage, p2, lane);
-            len = a.k_max;
+        if (fill > static_cast<uint32_t>(kStage)) fill = kStage;                     // (cannot happen: see the prune condition)
+        if (fill > a.k_max) {                             // S8: the K smallest keys
+            warp_select_keys(stage, fill, a.k_max, __float_as_uint(a.r2), lane, lt_mask);
+            fill = a.k_max;
         }
-        // ---- order the kept hits by dst: keys (j << 32 | d2 bits), second sort
+        const uint32_t len = fill;
+        // ---- order the kept hits by dst: keys (j << 32 | d2 bits), bitonic sort
         int p2 = 2;
         while (static_cast<uint32_t>(p2) < len) p2 <<= 1;
         for (int t = lane; t < p2; t += 32) {
@@ -1165,11 +1237,13 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     __shared__ uint32_t s_kept[kEmitThreads];              // medium rows: bit h set = stored hit h is among the K nearest
     __shared__ uint32_t s_mwarp[kEmitThreads / 32];
     __shared__ unsigned long long s_stage[kEmitThreads / 32][kStage];   // big rows: per-warp staging of (d2, j) keys
+    __shared__ unsigned int s_done;                        // timeline only: threads of the block that have finished
+    if (threadIdx.x == 0) s_done = 0u;                     // (made visible by the barriers below)
     stamp_begin(a.stamps, 4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t tile = blockIdx.x;
-    if (tile >= a.n_tiles) { stamp_end(a.stamps, 4); return; }
+    if (tile >= a.n_tiles) return;
     const int64_t tile_row0 = static_cast<int64_t>(tile) * kEmitThreads;
     const int64_t i = tile_row0 + threadIdx.x;
     const bool has = i < a.n_total;
@@ -1361,7 +1435,7 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
             else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], lane, lane_delta, lt_mask);
         }
     }
-    stamp_end(a.stamps, 4);
+    stamp_end_last(a.stamps, 4, &s_done);
 }
 
 }  // namespace frnn

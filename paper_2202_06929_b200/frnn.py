@@ -32,9 +32,18 @@ class FrnnOptions(_c.Structure):
 
 class FrnnGridReport(_c.Structure):
     """``frnn_grid_report`` of include/frnn.h (what frnn_suggest_grid saw and predicts)."""
-    _fields_ = [("grid_dims", _c.c_int32), ("grid_bits", _c.c_int32), ("reordered", _c.c_int32), ("sampled", _c.c_int64),
+    _fields_ = [("grid_dims", _c.c_int32), ("grid_bits", _c.c_int32), ("reordered", _c.c_int32), ("n_tried", _c.c_int32),
+                ("sampled", _c.c_int64),
                 ("predicted_candidates", _c.c_float), ("predicted_survivors", _c.c_float), ("predicted_us", _c.c_float),
-                ("extent_cells", _c.c_float * 16), ("pair_probability", _c.c_float * 16), ("key_probability", _c.c_float * 16)]
+                ("measured_us", _c.c_float),
+                ("extent_cells", _c.c_float * 16), ("pair_probability", _c.c_float * 16), ("key_probability", _c.c_float * 16),
+                ("tried_dims", _c.c_int32 * 12), ("tried_bits", _c.c_int32 * 12), ("tried_reordered", _c.c_int32 * 12),
+                ("tried_predicted_us", _c.c_float * 12), ("tried_measured_us", _c.c_float * 12)]
+
+    def tried(self):
+        """The measured shortlist as a list of dicts (empty when measure was off)."""
+        return [{"grid_dims": self.tried_dims[k], "grid_bits": self.tried_bits[k], "reordered": bool(self.tried_reordered[k]),
+                 "predicted_us": self.tried_predicted_us[k], "measured_us": self.tried_measured_us[k]} for k in range(self.n_tried)]
 
 
 FRNN_LAUNCH_DEFAULT, FRNN_LAUNCH_GRAPH, FRNN_LAUNCH_PLAIN = 0, 1, 2
@@ -56,7 +65,8 @@ _SIGNATURES = {
     "frnn_workspace_bytes_opt": (_c.c_size_t, [_OPT, _c.c_int64, _c.c_int, _c.c_int, _c.c_int]),
     "frnn_set_grid": (_c.c_int, [_c.c_int, _c.c_int]),
     "frnn_get_grid": (None, [_c.c_int64, _c.c_int, _c.c_int, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int)]),
-    "frnn_suggest_grid": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_int, _c.c_float, _OPT, _c.POINTER(FrnnGridReport), _c.c_void_p]),
+    "frnn_suggest_grid": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_int, _c.c_float, _c.c_int, _OPT, _c.POINTER(FrnnGridReport),
+                                     _c.c_void_p]),
     "frnn_build_opt": (_c.c_int, [_OPT] + _BUILD_ARGS),
     "frnn_build_batched_opt": (_c.c_int, [_OPT] + _BATCHED_ARGS),
     "frnn_host_pipeline_create_opt": (_c.c_int, [_OPT, _c.c_int64, _c.c_int, _c.c_int, _c.c_int64, _c.c_int, _c.POINTER(_c.c_void_p)]),
@@ -171,14 +181,15 @@ def frnn_get_grid(n_total: int, n_events: int = 1, dim: int = 8) -> tuple[int, i
 
 
 def frnn_suggest_grid(points: torch.Tensor, r: float, n_events: int = 1, opt: FrnnOptions | None = None,
-                      stream: torch.cuda.Stream | None = None) -> tuple[FrnnOptions, FrnnGridReport]:
-    """Data-driven choice of (grid_dims, grid_bits, order) for ``points`` (device, n x dim); synchronous."""
+                      stream: torch.cuda.Stream | None = None, measure: bool = False) -> tuple[FrnnOptions, FrnnGridReport]:
+    """Data-driven choice of (grid_dims, grid_bits, order) for ``points`` (device, n x dim); synchronous.
+    ``measure``: time the model's shortlist on the sample and take the fastest."""
     _require_cuda(points)
     n, dim = points.shape
     opt = opt if opt is not None else frnn_options()
     rep = FrnnGridReport()
     stream = stream or torch.cuda.current_stream(points.device)
-    _check(lib().frnn_suggest_grid(_ptr(points), n, int(n_events), dim, float(r), _c.byref(opt), _c.byref(rep),
+    _check(lib().frnn_suggest_grid(_ptr(points), n, int(n_events), dim, float(r), int(bool(measure)), _c.byref(opt), _c.byref(rep),
                                    _c.c_void_p(stream.cuda_stream)), "frnn_suggest_grid")
     return opt, rep
 

@@ -357,12 +357,23 @@ def test_suggested_grid_on_wide_offset_and_fine_data(F, extent, r, offset):
     exp = oracle.frnn(x, r, 32, oracle.CELLS)
     assert exp.count > 1000
     pts = torch.from_numpy(x).cuda()
-    opt, rep = F.frnn_suggest_grid(pts, r)
-    assert 1 <= opt.grid_dims <= 6 and 2 <= opt.grid_bits <= 8
-    assert (1 << (opt.grid_dims * opt.grid_bits)) <= 32 * n
-    ext = extent / (np.float32(r) * np.float32(1.0078125))
-    assert abs(rep.extent_cells[0] - ext) < 0.15 * ext + 2
-    for o in (opt, None):
+    tried_opts = [None]
+    for measure in (False, True):
+        opt, rep = F.frnn_suggest_grid(pts, r, measure=measure)
+        assert 1 <= opt.grid_dims <= 6 and 2 <= opt.grid_bits <= 8
+        assert (1 << (opt.grid_dims * opt.grid_bits)) <= 32 * n
+        ext = extent / (np.float32(r) * np.float32(1.0078125))
+        assert abs(rep.extent_cells[0] - ext) < 0.15 * ext + 2
+        if measure:
+            tried = rep.tried()
+            assert 1 <= len(tried) <= 12 and rep.measured_us > 0
+            assert rep.measured_us == min(t["measured_us"] for t in tried)         # the fastest of the shortlist was taken
+            assert any(t["grid_dims"] == opt.grid_dims and t["grid_bits"] == opt.grid_bits for t in tried)
+            print(f"[suggest] extent {extent} r {r}: ({opt.grid_dims},{opt.grid_bits}) {rep.measured_us:.1f} us of {tried}")
+        else:
+            assert rep.n_tried == 0
+        tried_opts.append(opt)
+    for o in tried_opts:
         res = F.frnn_build_ex(pts, r, 32, opt=o)
         torch.cuda.synchronize()
         res.check()
