@@ -132,7 +132,7 @@ void frnn_get_grid(int64_t n_total, int n_events, int dim, int* grid_dims, int* 
  * of the key filter that times the product of s(64 cells) over the keyed ones.  It then picks the (grid_dims,
  * grid_bits) -- and, only when that is predicted to gain more than 10 %, an order of the coordinates -- that minimise
  * a cost model of the path (fixed latency; table entries to zero and scan; per query: neighbour rows, keys, survivors;
- * constants in DESIGN.md section 7), over grids whose table stays within 32 cells per point of an event.
+ * constants in DESIGN.md section 7), over grids whose table stays within 64 cells per point of an event.
  *   measure == 0: the model's best is taken as it is (one small kernel, a stream synchronise).
  *   measure != 0: the model only makes a SHORTLIST (at most FRNN_GRID_REPORT_TRIES grids within 2.5x of its best); each
  *                 is then run for real on the first event of `points` (edge capacity 0: everything but the output

@@ -825,8 +825,8 @@ int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, flo
     const double n_event = static_cast<double>(n) / n_events;
     int ev_bits = 0;
     while ((1ll << ev_bits) < n_events) ++ev_bits;
-    // table budget: 32 cells per point of an event (a finer table costs more to zero and scan than it saves), 2^26 in all
-    const double budget = fmin(fmax(65536.0, 32.0 * n_event), 67108864.0 / n_events);
+    // table budget: 64 cells per point of an event (a finer table costs more to zero and scan than it saves), 2^26 in all
+    const double budget = fmin(fmax(65536.0, 64.0 * n_event), 67108864.0 / n_events);
     std::vector<GridTry> all;
     const bool same_order = memcmp(orders[0], orders[1], 8) == 0;
     for (int g = 1; g <= 6 && g <= dim; ++g)

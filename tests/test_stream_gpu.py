@@ -361,7 +361,7 @@ def test_suggested_grid_on_wide_offset_and_fine_data(F, extent, r, offset):
     for measure in (False, True):
         opt, rep = F.frnn_suggest_grid(pts, r, measure=measure)
         assert 1 <= opt.grid_dims <= 6 and 2 <= opt.grid_bits <= 8
-        assert (1 << (opt.grid_dims * opt.grid_bits)) <= 32 * n
+        assert (1 << (opt.grid_dims * opt.grid_bits)) <= 64 * n
         ext = extent / (np.float32(r) * np.float32(1.0078125))
         assert abs(rep.extent_cells[0] - ext) < 0.15 * ext + 2
         if measure:
