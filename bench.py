@@ -225,6 +225,7 @@ def main() -> None:
     ap.add_argument("--two-stream-steps", type=int, default=4000, help="steps of the two-events-in-flight throughput figure")
     ap.add_argument("--other-reps", type=int, default=50, help="repetitions for the other configs / N sweep / K and radius legs")
     ap.add_argument("--next-steps", type=int, default=300, help="timed repetitions of the two edge-list consumers")
+    ap.add_argument("--other-configs", default="0,1,3,4,sweep", help="which parts of the `other` leg run (for ncu captures of one config)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -582,7 +583,7 @@ def main() -> None:
                                  "note": "per edge: 8 B indices + 2 x 32 B rows read + 64 B written (streaming stores).  The row reads are served by L2 "
                                          "(one event = 3.84 MB), so the PHYSICAL DRAM traffic is the event once + indices + the written rows"},
             "label_components": {"us_per_event": l_us, "nodes": n, "edges": e_mean, "threshold": 0.5,
-                                 "components": int(ncomp.item()), "note": "3 kernels: init, hook (CAS union-find), flatten"},
+                                 "components": int(ncomp.item()), "note": "3 kernels (init, hook: CAS union-find, flatten) replayed as one graph"},
             "dense_bruteforce": {"ms_per_event": d_us * 1e-3, "pair_evaluations": n * (n - 1) / 2,
                                  "pairs_per_s": n * (n - 1) / 2 / (d_us * 1e-6), "slower_than_grid_path": d_us * 1e-3 / ms_per_step,
                                  "bound": "alu", "fp32_lane_instr_per_s": 16 * n * (n - 1) / 2 / (d_us * 1e-6),
@@ -598,7 +599,10 @@ def main() -> None:
     other = None
     if "other" in legs and args.other_reps > 0:
         other = {}
+        which = set(args.other_configs.split(","))
         for idx, reps in ((0, 20 * args.other_reps), (1, 20 * args.other_reps), (4, args.other_reps)):
+            if str(idx) not in which:
+                continue
             c = events.CONFIGS[idx]
             xe = events.make_event(c)
             ms_, e_, w_, p_ = time_single(xe, c.r, c.k_max, reps)
@@ -611,29 +615,31 @@ def main() -> None:
                 other[c.name].update({"timeline_us": tl, "roofline_issue": ri, "roofline_model": rm,
                                       "path_model_frac": (cand4 * 32.0 + 12.0 * e_) / (ms_ * 1e-3) / 1e9 / peak})
             del w_, p_
-        c3 = events.CONFIGS[3]
-        xb, offs = events.make_batch(c3)
-        pb = torch.from_numpy(xb).to(dev)
-        wb = F.Workspace(len(xb), c3.n_events, c3.k_max, len(xb) * 4, dev)
-        ms3 = timed(lambda i: F.frnn_build_batched(pb, offs, c3.r, c3.k_max, ws=wb, stream=stream), args.other_reps, warm=3)
-        assert int(wb.status.item()) == 0
-        e3 = int(wb.count[-1].item())
-        g3 = F.frnn_get_grid(len(xb), c3.n_events, 8)
-        tl3 = timeline_of(lambda i: F.frnn_build_batched(pb, offs, c3.r, c3.k_max, ws=wb, stream=stream), wb.buf, len(xb), c3.n_events,
-                          max(args.other_reps // 5, 2), group=2)
-        cand3 = sum(candidate_rows(xb[offs[e]:offs[e + 1]], c3.r, *g3) for e in range(2)) * c3.n_events / 2.0
-        ri3, rm3 = rooflines("cfg3", "search", tl3.get("search", {}).get("dur"), cand3 * 32.0 + 8.0 * e3)
-        other[c3.name] = {"n": len(xb), "events": c3.n_events, "ms_per_batch": ms3, "ms_per_event": ms3 / c3.n_events, "edges": e3,
-                          "edges_per_s": e3 / (ms3 * 1e-3), "grid": g3, "workspace_bytes": F.frnn_workspace_bytes(len(xb), c3.n_events, 8, c3.k_max),
-                          "timeline_us": tl3, "roofline_issue": ri3, "roofline_model": rm3,
-                          "path_model_frac": (cand3 * 32.0 + 12.0 * e3) / (ms3 * 1e-3) / 1e9 / peak}
-        del pb, wb
-        sweep = []
-        for nn in (15000, 30000, 60000, 120000):
-            c = dataclasses.replace(CFG, n=nn, n_tracks=CFG.n_tracks * nn // CFG.n)
-            ms_, e_, _, _ = time_single(events.make_event(c, 77), c.r, c.k_max, 10 * args.other_reps)
-            sweep.append({"n": nn, "ms_per_event": ms_, "edges": e_, "us_per_1k_points": 1e3 * ms_ / (nn / 1000)})
-        other["n_sweep_config2_recipe"] = sweep
+        if "3" in which:
+            c3 = events.CONFIGS[3]
+            xb, offs = events.make_batch(c3)
+            pb = torch.from_numpy(xb).to(dev)
+            wb = F.Workspace(len(xb), c3.n_events, c3.k_max, len(xb) * 4, dev)
+            ms3 = timed(lambda i: F.frnn_build_batched(pb, offs, c3.r, c3.k_max, ws=wb, stream=stream), args.other_reps, warm=3)
+            assert int(wb.status.item()) == 0
+            e3 = int(wb.count[-1].item())
+            g3 = F.frnn_get_grid(len(xb), c3.n_events, 8)
+            tl3 = timeline_of(lambda i: F.frnn_build_batched(pb, offs, c3.r, c3.k_max, ws=wb, stream=stream), wb.buf, len(xb), c3.n_events,
+                              max(args.other_reps // 5, 2), group=2)
+            cand3 = sum(candidate_rows(xb[offs[e]:offs[e + 1]], c3.r, *g3) for e in range(2)) * c3.n_events / 2.0
+            ri3, rm3 = rooflines("cfg3", "search", tl3.get("search", {}).get("dur"), cand3 * 32.0 + 8.0 * e3)
+            other[c3.name] = {"n": len(xb), "events": c3.n_events, "ms_per_batch": ms3, "ms_per_event": ms3 / c3.n_events, "edges": e3,
+                              "edges_per_s": e3 / (ms3 * 1e-3), "grid": g3, "workspace_bytes": F.frnn_workspace_bytes(len(xb), c3.n_events, 8, c3.k_max),
+                              "timeline_us": tl3, "roofline_issue": ri3, "roofline_model": rm3,
+                              "path_model_frac": (cand3 * 32.0 + 12.0 * e3) / (ms3 * 1e-3) / 1e9 / peak}
+            del pb, wb
+        if "sweep" in which:
+            sweep = []
+            for nn in (15000, 30000, 60000, 120000):
+                c = dataclasses.replace(CFG, n=nn, n_tracks=CFG.n_tracks * nn // CFG.n)
+                ms_, e_, _, _ = time_single(events.make_event(c, 77), c.r, c.k_max, 10 * args.other_reps)
+                sweep.append({"n": nn, "ms_per_event": ms_, "edges": e_, "us_per_1k_points": 1e3 * ms_ / (nn / 1000)})
+            other["n_sweep_config2_recipe"] = sweep
 
     # end to end through the host-buffer entry points: pinned host buffers, copies inside the timed region
     e2e = None

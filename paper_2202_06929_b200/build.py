@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfrnn_b200.so")
 SOURCES = [os.path.join(CSRC, "frnn.cu"), os.path.join(CSRC, "frnn_next.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "frnn_kernels.cuh"), os.path.join(HERE, "..", "include", "frnn.h")]
+DEPS = SOURCES + [os.path.join(CSRC, "frnn_kernels.cuh"), os.path.join(CSRC, "launch_plan.h"), os.path.join(HERE, "..", "include", "frnn.h")]
 # No --use_fast_math: the d2 chain is written with explicit rounding intrinsics and denormals must
 # not be flushed (R3).
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "--extended-lambda",

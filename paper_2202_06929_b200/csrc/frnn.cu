@@ -9,6 +9,7 @@
 // the pointers, r, k_max or the capacity, so a stream of events of different sizes replays ONE graph
 // (section 3: the latency "depends almost linearly on the number of spacepoints" -- events differ in size).
 #include "frnn_kernels.cuh"
+#include "launch_plan.h"
 
 #include <math.h>
 #include <stdio.h>
@@ -215,33 +216,7 @@ struct Call {                 // everything that determines the enqueued work
     Opts opts;
 };
 
-// ------------------------------------------------------------------------------------------------
-// The plan of a call
-// ------------------------------------------------------------------------------------------------
-struct Node {
-    const void* func;
-    unsigned grid_x, grid_y, block;
-    int phase;                    // kPhaseNames index (per-phase event timing)
-    uint32_t arg_off, arg_bytes;  // the by-value argument struct inside Plan::args
-};
-struct Plan {
-    void* ms_dst = nullptr;
-    size_t ms_bytes = 0;
-    std::vector<Node> nodes;
-    std::vector<unsigned char> args;
-    void clear() { ms_dst = nullptr; ms_bytes = 0; nodes.clear(); args.clear(); }
-    template <class A>
-    void add(const void* func, unsigned grid_x, unsigned grid_y, unsigned block, int phase, const A& a) {
-        static_assert(sizeof(A) <= 4096, "kernel arguments are limited to 4 KB");
-        const size_t off = (args.size() + 15) & ~static_cast<size_t>(15);
-        args.resize(off + sizeof(A));
-        memcpy(args.data() + off, &a, sizeof(A));
-        nodes.push_back(Node{func, grid_x, grid_y, block, phase, static_cast<uint32_t>(off), static_cast<uint32_t>(sizeof(A))});
-    }
-};
 thread_local Plan t_plan;         // reused: a call allocates nothing once the vectors have grown
-
-template <class K> const void* fptr(K k) { return reinterpret_cast<const void*>(k); }
 
 // The whole path as a plan.
 void make_plan(const Call& c, const Layout& L, Plan& P) {
@@ -343,8 +318,7 @@ int launch_plain(const Plan& P, cudaStream_t st) {
     const bool prof = g_profiling && g_ev_valid;
     int cur = 0;                                              // events recorded so far = cur + 1
     if (prof) cudaEventRecord(g_ev[0], st);
-    CK(cudaMemsetAsync(P.ms_dst, 0, P.ms_bytes, st));
-    ++t_launches;
+    if (P.ms_bytes) { CK(cudaMemsetAsync(P.ms_dst, 0, P.ms_bytes, st)); ++t_launches; }
     for (const Node& nd : P.nodes) {
         if (prof) for (; cur < nd.phase; ++cur) cudaEventRecord(g_ev[cur + 1], st);
         void* argp = const_cast<unsigned char*>(P.args.data() + nd.arg_off);
@@ -365,6 +339,7 @@ int launch_plain(const Plan& P, cudaStream_t st) {
 struct ExecEntry {
     void* workspace = nullptr;
     std::vector<const void*> funcs;
+    bool has_memset = true;
     cudaGraph_t graph = nullptr;  // kept alive: its node handles address the executable's nodes in the update calls
     cudaGraphExec_t exec = nullptr;
     cudaGraphNode_t ms_node = nullptr;
@@ -384,7 +359,7 @@ constexpr size_t kMaxExecs = 64;
 std::atomic<long long> g_graph_builds{0};     // frnn_graph_builds(): a stream of calls of one shape must not move it
 
 bool same_shape(const ExecEntry& e, const Plan& P) {
-    if (e.funcs.size() != P.nodes.size()) return false;
+    if (e.funcs.size() != P.nodes.size() || e.has_memset != (P.ms_bytes != 0)) return false;
     for (size_t k = 0; k < P.nodes.size(); ++k)
         if (e.funcs[k] != P.nodes[k].func) return false;
     return true;
@@ -418,15 +393,18 @@ int build_exec(ExecEntry& e, const Plan& P) {
     e.knodes.clear();
     cudaGraph_t graph = nullptr;
     CK(cudaGraphCreate(&graph, 0));
-    cudaError_t err;
-    const cudaMemsetParams mp = memset_params(P);
-    err = cudaGraphAddMemsetNode(&e.ms_node, graph, nullptr, 0, &mp);
-    cudaGraphNode_t prev = e.ms_node;
+    cudaError_t err = cudaSuccess;
+    cudaGraphNode_t prev = nullptr;
+    if (P.ms_bytes) {
+        const cudaMemsetParams mp = memset_params(P);
+        err = cudaGraphAddMemsetNode(&e.ms_node, graph, nullptr, 0, &mp);
+        prev = e.ms_node;
+    }
     for (size_t k = 0; err == cudaSuccess && k < P.nodes.size(); ++k) {
         void* argp = const_cast<unsigned char*>(P.args.data() + P.nodes[k].arg_off);
         const cudaKernelNodeParams kp = node_params(P.nodes[k], &argp);
         cudaGraphNode_t node = nullptr;
-        err = cudaGraphAddKernelNode(&node, graph, &prev, 1, &kp);
+        err = cudaGraphAddKernelNode(&node, graph, prev ? &prev : nullptr, prev ? 1 : 0, &kp);
         e.knodes.push_back(node);
         prev = node;
     }
@@ -440,7 +418,7 @@ int build_exec(ExecEntry& e, const Plan& P) {
 
 // write what changed since the last launch into the executable's nodes
 int update_exec(ExecEntry& e, const Plan& P) {
-    if (e.held.ms_dst != P.ms_dst || e.held.ms_bytes != P.ms_bytes) {
+    if (P.ms_bytes && (e.held.ms_dst != P.ms_dst || e.held.ms_bytes != P.ms_bytes)) {
         const cudaMemsetParams mp = memset_params(P);
         const cudaError_t err = cudaGraphExecMemsetNodeSetParams(e.exec, e.ms_node, &mp);
         if (err != cudaSuccess) return cuda_fail(err, "cudaGraphExecMemsetNodeSetParams");
@@ -479,6 +457,7 @@ int launch_graph(const Plan& P, void* workspace, cudaStream_t st) {
             }
             e = std::make_shared<ExecEntry>();
             e->workspace = workspace;
+            e->has_memset = P.ms_bytes != 0;
             for (const Node& nd : P.nodes) e->funcs.push_back(nd.func);
             g_execs.push_back(e);
         }
@@ -490,9 +469,27 @@ int launch_graph(const Plan& P, void* workspace, cudaStream_t st) {
     else if ((rc = update_exec(*e, P)) != FRNN_OK) rc = build_exec(*e, P);     // an update the driver refuses: start over (counted, see frnn_graph_builds)
     if (rc != FRNN_OK) return rc;
     CK(cudaGraphLaunch(e->exec, st));
-    t_launches = static_cast<int>(P.nodes.size()) + 1;
+    t_launches = static_cast<int>(P.nodes.size()) + (P.ms_bytes ? 1 : 0);
     return FRNN_OK;
 }
+
+}  // namespace
+
+namespace frnn {
+int run_plan(const Plan& P, void* key, cudaStream_t st, bool want_graph) {
+    t_launches = 0;
+    bool graph_ok = want_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
+    if (graph_ok) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); graph_ok = false; }   // caller is capturing: just enqueue
+    }
+    if (!graph_ok) return launch_plain(P, st);
+    return launch_graph(P, key, st);
+}
+bool default_use_graph() { return default_opts().use_graph; }
+}  // namespace frnn
+
+namespace {
 
 int run_call(const Call& c, cudaStream_t st) {
     t_launches = 0;
@@ -507,13 +504,7 @@ int run_call(const Call& c, cudaStream_t st) {
     const Layout L = make_layout(n_total, c.n_events, GridChoice{c.grid_dims, c.grid_bits}, c.dim, c.opts.order.on != 0);
     Plan& P = t_plan;
     make_plan(c, L, P);
-    bool graph_ok = c.opts.use_graph && !g_profiling && st != nullptr && st != cudaStreamLegacy;
-    if (graph_ok) {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { cudaGetLastError(); graph_ok = false; }   // caller is capturing: just enqueue
-    }
-    if (!graph_ok) return launch_plain(P, st);
-    return launch_graph(P, c.workspace, st);
+    return frnn::run_plan(P, c.workspace, st, c.opts.use_graph);
 }
 
 int prepare(Call& c, size_t workspace_bytes) {

@@ -9,6 +9,7 @@
 #include <stdint.h>
 
 #include "../../include/frnn.h"
+#include "launch_plan.h"
 
 namespace {
 
@@ -52,10 +53,22 @@ __global__ void __launch_bounds__(256) gather_edge_rows_kernel(const float4* __r
 // f2: lock-free union-find.  parent[] lives in `labels`.  A root is only ever linked to a SMALLER index, so the
 // root of a tree is the smallest index of its component and the final label is canonical.
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) cc_init_kernel(int32_t* __restrict__ parent, int64_t n, int32_t* __restrict__ n_components) {
+// (one by-value argument struct per kernel: the three launches are the nodes of a cached CUDA graph, see launch_plan.h)
+struct CcArgs {
+    int32_t* parent;
+    int64_t n;
+    const int32_t* src;
+    const int32_t* dst;
+    const float* score;
+    float threshold;
+    const int64_t* edge_count;
+    int64_t edge_max;
+    int32_t* n_components;
+};
+__global__ void __launch_bounds__(256) cc_init_kernel(CcArgs a) {
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < n) parent[i] = static_cast<int32_t>(i);
-    if (i == 0 && n_components) *n_components = 0;
+    if (i < a.n) a.parent[i] = static_cast<int32_t>(i);
+    if (i == 0 && a.n_components) *a.n_components = 0;
 }
 
 // find with path halving, starting from x whose parent px has already been loaded (L2-coherent loads: other blocks
@@ -70,11 +83,15 @@ __device__ __forceinline__ int32_t cc_find(int32_t* parent, int32_t x, int32_t p
     return x;
 }
 
-__global__ void __launch_bounds__(256) cc_hook_kernel(int32_t* __restrict__ parent, int64_t n,
-                                                      const int32_t* __restrict__ src, const int32_t* __restrict__ dst,
-                                                      const float* __restrict__ score, float threshold,
-                                                      const int64_t* __restrict__ edge_count, int64_t edge_max) {
-    int64_t e_end = edge_max;
+__global__ void __launch_bounds__(256) cc_hook_kernel(CcArgs a) {
+    int32_t* __restrict__ parent = a.parent;
+    const int64_t n = a.n;
+    const int32_t* __restrict__ src = a.src;
+    const int32_t* __restrict__ dst = a.dst;
+    const float* __restrict__ score = a.score;
+    const float threshold = a.threshold;
+    const int64_t* __restrict__ edge_count = a.edge_count;
+    int64_t e_end = a.edge_max;
     if (edge_count) { const int64_t c = *edge_count; e_end = c < e_end ? c : e_end; }
     for (int64_t e = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x; e < e_end;
          e += static_cast<int64_t>(gridDim.x) * blockDim.x) {
@@ -98,7 +115,10 @@ __global__ void __launch_bounds__(256) cc_hook_kernel(int32_t* __restrict__ pare
     }
 }
 
-__global__ void __launch_bounds__(256) cc_flatten_kernel(int32_t* __restrict__ parent, int64_t n, int32_t* __restrict__ n_components) {
+__global__ void __launch_bounds__(256) cc_flatten_kernel(CcArgs a) {
+    int32_t* __restrict__ parent = a.parent;
+    const int64_t n = a.n;
+    int32_t* __restrict__ n_components = a.n_components;
     const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     bool root = false;
     if (i < n) {
@@ -157,11 +177,15 @@ int frnn_label_components(int64_t n, const int32_t* src, const int32_t* dst, con
         if (n_components && cudaMemsetAsync(n_components, 0, 4, st) != cudaSuccess) return FRNN_ERR_CUDA;
         return FRNN_OK;
     }
-    cc_init_kernel<<<blocks_for(n, 256, 0x7fffffff), 256, 0, st>>>(labels, n, n_components);
-    if (edge_max > 0)
-        cc_hook_kernel<<<blocks_for(edge_max, 256, 148 * 64), 256, 0, st>>>(labels, n, src, dst, score, threshold, edge_count, edge_max);
-    cc_flatten_kernel<<<blocks_for(n, 256, 0x7fffffff), 256, 0, st>>>(labels, n, n_components);
-    return cudaGetLastError() == cudaSuccess ? FRNN_OK : FRNN_ERR_CUDA;
+    // the three kernels as a plan: on a non-default stream they replay the graph that belongs to the labels array
+    // (node parameters rewritten when the edge list or the threshold changed), else they are launched one by one
+    thread_local frnn::Plan plan;
+    plan.clear();
+    const CcArgs a{labels, n, src, dst, score, threshold, edge_count, edge_max, n_components};
+    plan.add(frnn::fptr(cc_init_kernel), blocks_for(n, 256, 0x7fffffff), 1, 256, 0, a);
+    if (edge_max > 0) plan.add(frnn::fptr(cc_hook_kernel), blocks_for(edge_max, 256, 148 * 64), 1, 256, 0, a);
+    plan.add(frnn::fptr(cc_flatten_kernel), blocks_for(n, 256, 0x7fffffff), 1, 256, 0, a);
+    return frnn::run_plan(plan, labels, st, frnn::default_use_graph());
 }
 
 }  // extern "C"
