@@ -501,7 +501,10 @@ constexpr int kSearchThreads = 128;
 constexpr int kBatch = FRNN_KBATCH;    // candidates of a run tested per batch
 constexpr int kQueue = 32;             // survivor queue entries per thread (>= 2 * 3 * kBatch)
 constexpr int kLeft = 15;              // leftover-run entries per thread (the runs of 5 sub-batches)
-constexpr int kSlot = 32;              // hit slots per row in the scratch buffer
+constexpr int kSlot = 32;              // hit slots per row in the scratch buffer: 256 B per row reserved, one 32-byte sector touched per 4
+                                       // hits.  Smaller layouts were built and measured in round 2 (profiles/r02_summary.md): 16 slots cost
+                                       // 3 us per event (the 10 rows in 120,000 with more hits are recomputed by a warp, ~3 us each, at the
+                                       // end of emit); 4 inline slots + a per-tile overflow pool cost 9 us (same-address returning atomics)
 #ifndef FRNN_EMIT_THREADS
 #define FRNN_EMIT_THREADS 256
 #endif

@@ -156,13 +156,13 @@ def test_plain_launch_mode_and_graph_mode_agree(F):
 
 
 # ---------------------------------------------------------------- item 2: S8 when K binds
-@pytest.mark.parametrize("k", [1, 5, 31, 32, 33, 64])
+@pytest.mark.parametrize("k", [1, 5, 15, 16, 17, 31, 32, 33, 64])
 def test_counts_straddling_the_slot_buffer(F, k):
-    """Rows with 24..44 neighbours (cluster sizes 25..45): counts on both sides of the 32 hit slots, K on both sides of
-    the counts -- small, medium (from the slot buffer) and big (recomputed, staged, selected) rows in the same tiles."""
-    x = tight_clusters(list(range(25, 46)) * 3, 5)
+    """Rows with 7..44 neighbours (cluster sizes 8..45): counts on both sides of the 32 hit slots per row (and of 16, a layout that was tried), K on
+    both sides of the counts -- small, medium (from the slot buffer) and big (recomputed, staged, selected) rows in the same tiles."""
+    x = tight_clusters(list(range(8, 46)) * 2, 5)
     exp = oracle.frnn(x, 0.1, k, oracle.BRUTE)
-    assert exp.uncapped.min() == 24 and exp.uncapped.max() == 44
+    assert exp.uncapped.min() == 7 and exp.uncapped.max() == 44
     res = F.frnn_build_ex(torch.from_numpy(x).cuda(), 0.1, k)
     torch.cuda.synchronize()
     res.check()
