@@ -259,8 +259,10 @@ void make_plan(const Call& c, const Layout& L, Plan& P) {
         DenseArgs da;
         da.pts = pts; da.dim = c.dim; da.cnt = cnt; da.hits = hits; da.tile_deg = tile_deg; da.n_tiles = emit_tiles;
         da.n = n_total; da.r2 = r2; da.k_max = static_cast<uint32_t>(c.k_max);
-        const unsigned T = static_cast<unsigned>((n_total + kDenseTile - 1) / kDenseTile);
-        P.add(c.dim > kDim ? fptr(dense_search_kernel<true>) : fptr(dense_search_kernel<false>), T, T, kDenseTile, 4, da);
+        const unsigned T = static_cast<unsigned>((n_total + kDenseTile - 1) / kDenseTile);              // candidate tiles (x)
+        const int qrows = (c.dim > kDim ? DenseCfg<true>::Q : DenseCfg<false>::Q) * kDenseTile;          // queries per block (y)
+        const unsigned TQ = static_cast<unsigned>((n_total + qrows - 1) / qrows);
+        P.add(c.dim > kDim ? fptr(dense_search_kernel<true>) : fptr(dense_search_kernel<false>), T, TQ, kDenseTile, 4, da);
         ea.spts = nullptr; ea.spts_hi = nullptr; ea.sidx = nullptr; ea.cell_start = nullptr; ea.ev_off = nullptr; ea.n_events = 1;
         ea.out_edge_offsets = nullptr; ea.stamps = nullptr; ea.dense = 1;
         if (L.emit_tiles > kPrefixTilesMin) {

@@ -840,20 +840,72 @@ struct DenseArgs {
     uint32_t k_max;
 };
 
+// Register tiling: a thread holds kDenseQ queries (kDenseQ x 8 floats) and runs their chains against every candidate row
+// it reads from shared memory, so the two 128-bit shared loads of a candidate (broadcasts: all lanes read the same row) are
+// paid once per kDenseQ pairs -- 16 kDenseQ FP32 instructions per 2 loads instead of 16.  Block (I, J): queries
+// [I * kDenseQ * 128, +kDenseQ * 128) x candidates [J * 128, +128); blocks entirely below the diagonal leave at once, blocks
+// on it test j > i per pair.
+template <bool HI> struct DenseCfg { static constexpr int Q = HI ? 2 : 4; };
+
+// a hit of the brute-force search (rare: kept out of line so that the pair loop stays tight)
+__device__ __noinline__ void dense_hit(const DenseArgs& a, unsigned long long* my_tile_deg, int32_t row, int32_t cj, float d2) {
+    const int d2b = __float_as_int(d2);
+    const uint32_t p0 = atomicAdd(&a.cnt[row], 1u);
+    const uint32_t p1 = atomicAdd(&a.cnt[cj], 1u);
+    if (p0 < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + p0] = make_int2(cj, d2b);
+    if (p1 < kSlot) a.hits[static_cast<int64_t>(cj) * kSlot + p1] = make_int2(row, d2b);
+    if (p0 < a.k_max) atomicAdd(&my_tile_deg[row / kEmitThreads], 1ull);
+    if (p1 < a.k_max) atomicAdd(&my_tile_deg[cj / kEmitThreads], 1ull);
+}
+
+template <bool HI, bool DIAG, int Q>
+__device__ __forceinline__ void dense_pairs(const DenseArgs& a, const float4 (*s_c)[HI ? 4 : 2], const float4* qa, const float4* qb,
+                                            const float4* qc, const float4* qd, const int* qrel, int64_t q_lo, int64_t c_lo,
+                                            unsigned long long* my_tile_deg, int tid) {
+#pragma unroll 4
+    for (int k = 0; k < kDenseTile; ++k) {
+        const float4 ka = s_c[k][0], kb = s_c[k][1];
+        float d2[Q];
+#pragma unroll
+        for (int q = 0; q < Q; ++q) d2[q] = d2_pinned(qa[q], qb[q], ka, kb);
+        if (HI) {
+            const float4 kc = s_c[k][2], kd = s_c[k][3];
+#pragma unroll
+            for (int q = 0; q < Q; ++q) d2[q] = d2_continue(d2[q], qc[q], qd[q], kc, kd);
+        }
+#pragma unroll
+        for (int q = 0; q < Q; ++q)
+            if (d2[q] <= a.r2 && (!DIAG || k > qrel[q]))
+                dense_hit(a, my_tile_deg, static_cast<int32_t>(q_lo + q * kDenseTile + tid), static_cast<int32_t>(c_lo + k), d2[q]);
+    }
+}
+
 template <bool HI>
 __global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
+    constexpr int Q = DenseCfg<HI>::Q;
     const uint32_t I = blockIdx.y, J = blockIdx.x;
-    if (J < I) return;
+    const int64_t q_lo = static_cast<int64_t>(I) * Q * kDenseTile;            // first query of the block
+    const int64_t c_lo = static_cast<int64_t>(J) * kDenseTile;                // first candidate of the block
+    if (c_lo + kDenseTile - 1 <= q_lo) return;                                // every candidate <= every query: nothing forward
     __shared__ float4 s_c[kDenseTile][HI ? 4 : 2];
     const int tid = threadIdx.x;
-    const int64_t i = static_cast<int64_t>(I) * kDenseTile + tid;
-    const int64_t jr = static_cast<int64_t>(J) * kDenseTile + tid;
-    float4 qa = make_float4(0.f, 0.f, 0.f, 0.f), qb = qa, qc = qa, qd = qa;
-    if (i < a.n) {
-        load_point(a.pts, i, a.dim, qa, qb);
-        if (HI) load_point_hi(a.pts, i, a.dim, qc, qd);
+    const float inf = __int_as_float(0x7f800000);
+    float4 qa[Q], qb[Q], qc[Q], qd[Q];
+    int qrel[Q];                                                              // query index relative to the first candidate (diagonal blocks)
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        const int64_t qi = q_lo + q * kDenseTile + tid;
+        const int64_t rel = qi - c_lo;
+        qrel[q] = rel < -1 ? -1 : (rel > kDenseTile ? kDenseTile : static_cast<int>(rel));
+        qa[q] = make_float4(-inf, 0.f, 0.f, 0.f);                             // queries beyond the event: -inf, never within r of anything
+        qb[q] = make_float4(0.f, 0.f, 0.f, 0.f); qc[q] = qb[q]; qd[q] = qb[q];
+        if (qi < a.n) {
+            load_point(a.pts, qi, a.dim, qa[q], qb[q]);
+            if (HI) load_point_hi(a.pts, qi, a.dim, qc[q], qd[q]);
+        }
     }
-    float4 ca = make_float4(__int_as_float(0x7f800000), 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f), cc = cb, cd = cb;
+    const int64_t jr = c_lo + tid;
+    float4 ca = make_float4(inf, 0.f, 0.f, 0.f), cb = make_float4(0.f, 0.f, 0.f, 0.f), cc = cb, cd = cb;
     if (jr < a.n) {                                                     // rows beyond the event: +inf, never within r
         load_point(a.pts, jr, a.dim, ca, cb);
         if (HI) load_point_hi(a.pts, jr, a.dim, cc, cd);
@@ -861,25 +913,11 @@ __global__ void __launch_bounds__(kDenseTile) dense_search_kernel(DenseArgs a) {
     s_c[tid][0] = ca; s_c[tid][1] = cb;
     if (HI) { s_c[tid][2] = cc; s_c[tid][3] = cd; }
     __syncthreads();
-    if (i >= a.n) return;
     unsigned long long* const my_tile_deg = a.tile_deg + static_cast<size_t>(J & (kDegSlices - 1)) * a.n_tiles;
-    const int k0 = I == J ? tid + 1 : 0;                               // own tile: only the rows after mine
-    const int32_t row = static_cast<int32_t>(i);
-#pragma unroll 4
-    for (int k = k0; k < kDenseTile; ++k) {
-        float d2 = d2_pinned(qa, qb, s_c[k][0], s_c[k][1]);
-        if (HI) d2 = d2_continue(d2, qc, qd, s_c[k][2], s_c[k][3]);
-        if (d2 <= a.r2) {
-            const int32_t cj = static_cast<int32_t>(J * kDenseTile + k);
-            const int d2b = __float_as_int(d2);
-            const uint32_t p0 = atomicAdd(&a.cnt[row], 1u);
-            const uint32_t p1 = atomicAdd(&a.cnt[cj], 1u);
-            if (p0 < kSlot) a.hits[static_cast<int64_t>(row) * kSlot + p0] = make_int2(cj, d2b);
-            if (p1 < kSlot) a.hits[static_cast<int64_t>(cj) * kSlot + p1] = make_int2(row, d2b);
-            if (p0 < a.k_max) atomicAdd(&my_tile_deg[row / kEmitThreads], 1ull);
-            if (p1 < a.k_max) atomicAdd(&my_tile_deg[cj / kEmitThreads], 1ull);
-        }
-    }
+    if (c_lo < q_lo + Q * kDenseTile)                                         // some candidate index <= some query index: test j > i per pair
+        dense_pairs<HI, true, Q>(a, s_c, qa, qb, qc, qd, qrel, q_lo, c_lo, my_tile_deg, tid);
+    else
+        dense_pairs<HI, false, Q>(a, s_c, qa, qb, qc, qd, qrel, q_lo, c_lo, my_tile_deg, tid);
 }
 
 // ------------------------------------------------------------------------------------------------
