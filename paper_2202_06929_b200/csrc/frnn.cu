@@ -559,6 +559,28 @@ size_t workspace_bytes_for(const Opts& o, int64_t n_total, int n_events, int dim
     return make_layout(n_total, n_events, choose_grid(o, n_total, n_events, dim), dim, o.order.on != 0).total;
 }
 
+// The three edge arrays to the host.  On the device they sit one capacity apart; when the caller's three host arrays are
+// equally spaced too (one block holding src | dst | d2, the natural way to allocate them) they travel as ONE 2-D copy of
+// three rows -- a DMA set-up costs about 6 us, and three copies per event instead of one cost 17 us of a 100 us event
+// (profiles/r02_summary.md); otherwise as three copies.
+// (Equally spaced arrays that are SEPARATE page-locked allocations make the runtime refuse the 2-D copy; *refused remembers
+// the base pointer for which that happened, so that it is not tried again for the same buffers.)
+int copy_edges_to_host(int32_t* h_src, int32_t* h_dst, float* h_d2, const int32_t* d_src, size_t d_cap, size_t e, cudaStream_t st,
+                       const void** refused) {
+    if (!e) return FRNN_OK;
+    const ptrdiff_t p1 = reinterpret_cast<char*>(h_dst) - reinterpret_cast<char*>(h_src);
+    const ptrdiff_t p2 = reinterpret_cast<char*>(h_d2) - reinterpret_cast<char*>(h_dst);
+    if (p1 == p2 && p1 >= static_cast<ptrdiff_t>(e * 4) && *refused != h_src) {
+        if (cudaMemcpy2DAsync(h_src, static_cast<size_t>(p1), d_src, d_cap * 4, e * 4, 3, cudaMemcpyDeviceToHost, st) == cudaSuccess) return FRNN_OK;
+        cudaGetLastError();
+        *refused = h_src;
+    }
+    CK(cudaMemcpyAsync(h_src, d_src, e * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_dst, d_src + d_cap, e * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h_d2, d_src + 2 * d_cap, e * 4, cudaMemcpyDeviceToHost, st));
+    return FRNN_OK;
+}
+
 // cached device buffers for the synchronous convenience entry points (one user at a time: g_cache_mutex)
 struct Cache {
     void* ws = nullptr; size_t ws_bytes = 0;
@@ -1032,9 +1054,8 @@ int frnn_build_host(const float* points, int64_t n, int dim, float r, int k_max,
     if (*out_count > edge_capacity) return FRNN_ERR_CAPACITY;
     const size_t e = static_cast<size_t>(*out_count);
     if (e) {
-        CK(cudaMemcpyAsync(out_src, d_src, e * 4, cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync(out_dst, d_dst, e * 4, cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync(out_d2, d_d2, e * 4, cudaMemcpyDeviceToHost, st));
+        static const void* refused = nullptr;                     // (under g_cache_mutex)
+        if ((rc = copy_edges_to_host(out_src, out_dst, out_d2, d_src, g_cache.edge_cap, e, st, &refused)) != FRNN_OK) return rc;
         CK(cudaStreamSynchronize(st));
     }
     return FRNN_OK;
@@ -1053,6 +1074,7 @@ struct frnn_host_pipeline {
         int64_t* count = nullptr;                                 // device: count (8 bytes) followed by status (4 bytes)
         int64_t* pinned = nullptr;                                // page-locked mirror of the two words above
         int32_t* h_src = nullptr; int32_t* h_dst = nullptr; float* h_d2 = nullptr; int64_t* h_count = nullptr;   // the caller's
+        const void* refused_2d = nullptr;                         // see copy_edges_to_host
         State state = FREE;
     };
     std::vector<Slot> slots;
@@ -1085,11 +1107,8 @@ int pipeline_start_copy(frnn_host_pipeline* p, frnn_host_pipeline::Slot& s) {
     const int32_t status = *reinterpret_cast<const int32_t*>(s.pinned + 1);
     *s.h_count = status == 0 ? c : -c - 1;                       // negative: capacity exceeded, -(needed) - 1
     const size_t e = static_cast<size_t>(c < p->cap ? c : p->cap);
-    if (e) {
-        CK(cudaMemcpyAsync(s.h_src, s.src, e * 4, cudaMemcpyDeviceToHost, s.stream));
-        CK(cudaMemcpyAsync(s.h_dst, s.dst, e * 4, cudaMemcpyDeviceToHost, s.stream));
-        CK(cudaMemcpyAsync(s.h_d2, s.d2, e * 4, cudaMemcpyDeviceToHost, s.stream));
-    }
+    const int crc = copy_edges_to_host(s.h_src, s.h_dst, s.h_d2, s.src, static_cast<size_t>(p->cap), e, s.stream, &s.refused_2d);
+    if (crc != FRNN_OK) return crc;
     CK(cudaEventRecord(s.done, s.stream));
     s.state = frnn_host_pipeline::COPYING;
     return FRNN_OK;

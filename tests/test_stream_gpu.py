@@ -274,11 +274,14 @@ def test_host_pipeline_at_tracking_scale_with_ragged_events(F):
     xs = [np.ascontiguousarray(full[i % 3][:m]) for i, m in enumerate(sizes)]
     pins = [torch.from_numpy(x).pin_memory() for x in xs]
 
-    def bufs(pinned):
+    def bufs(pinned, packed):
         mk = (lambda t: t.pin_memory()) if pinned else (lambda t: t)
+        if packed:                                         # src | dst | d2 in one block: the library sends them as one 2-D copy
+            blk = mk(torch.empty(3 * cap + 64, dtype=torch.int32))
+            return blk[:cap], blk[cap + 32:2 * cap + 32], blk[2 * cap + 64:].view(torch.float32), mk(torch.zeros(1, dtype=torch.int64))
         return (mk(torch.empty(cap, dtype=torch.int32)), mk(torch.empty(cap, dtype=torch.int32)), mk(torch.empty(cap, dtype=torch.float32)),
                 mk(torch.zeros(1, dtype=torch.int64)))
-    outs = [bufs(pinned=(i % 4 != 3)) for i in range(12)]
+    outs = [bufs(pinned=(i % 4 != 3), packed=(i % 3 != 0)) for i in range(12)]
     for p, o in zip(pins, outs):
         pipe.submit(p, cfg.r, *o)
     pipe.wait()
@@ -298,6 +301,10 @@ def test_build_host_at_tracking_scale_and_unaligned_host_rows(F):
     hs, hd, hq = torch.empty(cap, dtype=torch.int32), torch.empty(cap, dtype=torch.int32), torch.empty(cap, dtype=torch.float32)
     e = F.frnn_build_host(torch.from_numpy(x), cfg.r, cfg.k_max, hs, hd, hq)
     assert_same(Got(hs[:e].numpy(), hd[:e].numpy(), hq[:e].numpy()), exp, cfg.r, "frnn_build_host 120k")
+    blk = torch.empty(3 * cap, dtype=torch.int32).pin_memory()         # equally spaced outputs: one 2-D copy
+    ps, pd, pq = blk[:cap], blk[cap:2 * cap], blk[2 * cap:].view(torch.float32)
+    e = F.frnn_build_host(torch.from_numpy(x).pin_memory(), cfg.r, cfg.k_max, ps, pd, pq)
+    assert_same(Got(ps[:e].numpy(), pd[:e].numpy(), pq[:e].numpy()), exp, cfg.r, "frnn_build_host 120k, packed outputs")
     # a host array whose rows start 4 bytes past a 32-byte boundary: only the device fast path needs the alignment
     raw = torch.empty(cfg.n * 8 + 16, dtype=torch.float32)
     off = 1 + (-(raw.data_ptr() // 4)) % 8
