@@ -80,7 +80,13 @@ const char* frnn_last_error_string(void);
  * dimensions" of the embedding and notes that the cost of the cells grows as O(3^k k n) with the number k of binned
  * coordinates; which and how many coordinates are binned, and how many cells the toroidal grid has per coordinate,
  * never change the RESULT (R8/R9), only the amount of pruning and the size of the cell table.
- *   grid_dims   number of binned coordinates, 1..6; 0 = automatic (from the event size)
+ *   grid_dims   number of binned coordinates, 1..6; 0 = from the event size alone (no look at the data, no synchronisation);
+ *               FRNN_GRID_AUTO (-1) = chosen PER CALL from the call's own rows: the call first runs the estimate of
+ *               frnn_suggest_grid (measure = 0: cell histograms of a sample, cost model, default coordinate order) on
+ *               cuda_stream and SYNCHRONISES that stream once (about 60 us), then enqueues the build on the grid it picked;
+ *               grid_bits is ignored; the workspace must hold frnn_workspace_bytes_opt() with the same options (room for any
+ *               grid the call may pick).  For streams whose statistics really change from event to event; otherwise choose
+ *               once with frnn_suggest_grid and reuse the options.
  *   grid_bits   log2 of the toroidal grid extent per binned coordinate, 2..8; 0 = automatic (5).  With fewer cells
  *               than the data's extent / r, far-apart cells alias onto one table entry: exact, more candidates.
  *   order       order[0..order_count) = coordinates (0..15, distinct) binned first and keyed next, as in
@@ -90,6 +96,7 @@ const char* frnn_last_error_string(void);
  * struct_bytes must be sizeof(frnn_options) of the caller's header (frnn_options_init sets it).
  */
 enum { FRNN_LAUNCH_DEFAULT = 0, FRNN_LAUNCH_GRAPH = 1, FRNN_LAUNCH_PLAIN = 2 };
+enum { FRNN_GRID_AUTO = -1 };
 typedef struct frnn_options {
     uint32_t struct_bytes;
     int32_t grid_dims;

@@ -48,7 +48,8 @@ int cuda_fail(cudaError_t e, const char* what) {
 // ---- per-call options; the process-wide defaults (frnn_set_grid / _bin_order / _graph_mode / _profiling(2)) are
 // snapshotted once per call under a mutex, so concurrent calls never see a half-written default
 struct Opts {
-    int grid_dims = 0, grid_bits = 0;       // 0 = automatic
+    int grid_dims = 0, grid_bits = 0;       // 0 = from the event size
+    bool auto_grid = false;                 // FRNN_GRID_AUTO: the call looks at its own event first (one stream synchronise)
     BinOrder order = {0, {0, 1, 2, 3, 4, 5, 6, 7}};
     bool use_graph = true;
     bool timeline = false;
@@ -86,10 +87,11 @@ int opts_from(const frnn_options* in, Opts* out) {
     Opts o = default_opts();
     if (in) {
         if (in->struct_bytes < sizeof(frnn_options)) return FRNN_ERR_INVALID_ARG;
-        if (in->grid_dims < 0 || in->grid_dims > 6 || (in->grid_bits != 0 && (in->grid_bits < 2 || in->grid_bits > 8))) return FRNN_ERR_INVALID_ARG;
+        if (in->grid_dims < FRNN_GRID_AUTO || in->grid_dims > 6 || (in->grid_bits != 0 && (in->grid_bits < 2 || in->grid_bits > 8))) return FRNN_ERR_INVALID_ARG;
         if (in->launch_mode < 0 || in->launch_mode > 2) return FRNN_ERR_INVALID_ARG;
-        o.grid_dims = in->grid_dims;
-        o.grid_bits = in->grid_bits;
+        o.auto_grid = in->grid_dims == FRNN_GRID_AUTO;
+        o.grid_dims = o.auto_grid ? 0 : in->grid_dims;
+        o.grid_bits = o.auto_grid ? 0 : in->grid_bits;
         const int rc = make_order(in->order, in->order_count, &o.order);
         if (rc != FRNN_OK) return rc;
         if (in->launch_mode == FRNN_LAUNCH_GRAPH) o.use_graph = true;
@@ -521,6 +523,16 @@ int prepare(Call& c, size_t workspace_bytes) {
     return FRNN_OK;
 }
 
+// table budget of the data-driven choices: 64 cells per point of an event (a finer table costs more to zero and scan than
+// it saves), 2^26 cells in all, and a linear cell id that fits 30 bits
+bool grid_within_budget(int g, int bits, double n_event, int n_events) {
+    int ev_bits = 0;
+    while ((1ll << ev_bits) < n_events) ++ev_bits;
+    const double budget = fmin(fmax(65536.0, 64.0 * n_event), 67108864.0 / n_events);
+    return g * bits + ev_bits <= 30 && pow(2.0, g * bits) <= budget;
+}
+int auto_grid(const float* points, int64_t n, int n_events, int dim, float r, cudaStream_t st, int* g, int* bits);   // below
+
 int build_single(const Opts& o, bool dense, const float* points, int64_t n, int dim, float r, int k_max,
                  int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
                  int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr,
@@ -533,6 +545,10 @@ int build_single(const Opts& o, bool dense, const float* points, int64_t n, int 
     Call c{points, dim, 1, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, nullptr, out_status, out_row_ptr, workspace, 0, 0, ev_off};
     c.dense = dense;
     c.opts = o;
+    if (o.auto_grid && !dense && n > 0) {                                     // S1 from this very event (synchronises the stream once)
+        c.opts.auto_grid = false;
+        if ((rc = auto_grid(points, n, 1, dim, r, static_cast<cudaStream_t>(cuda_stream), &c.opts.grid_dims, &c.opts.grid_bits)) != FRNN_OK) return rc;
+    }
     if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
     return run_call(c, static_cast<cudaStream_t>(cuda_stream));
 }
@@ -550,12 +566,29 @@ int build_batched(const Opts& o, const float* points, const int64_t* event_offse
     Call c{points, dim, n_events, r, k_max, out_src, out_dst, out_d2, edge_capacity, nullptr, out_edge_offsets, out_status, out_row_ptr,
            workspace, 0, 0, event_offsets};
     c.opts = o;
+    if (o.auto_grid && event_offsets[n_events] > 0) {
+        c.opts.auto_grid = false;
+        if ((rc = auto_grid(points, event_offsets[n_events], n_events, dim, r, static_cast<cudaStream_t>(cuda_stream), &c.opts.grid_dims,
+                            &c.opts.grid_bits)) != FRNN_OK) return rc;
+    }
     if ((rc = prepare(c, workspace_bytes)) != FRNN_OK) return rc;
     return run_call(c, static_cast<cudaStream_t>(cuda_stream));
 }
 
 size_t workspace_bytes_for(const Opts& o, int64_t n_total, int n_events, int dim, int k_max) {
     if (n_total < 0 || n_events < 1 || dim < 1 || dim > kDimMax || k_max < 1 || n_total > 0x7fffffffll) return 0;
+    if (o.auto_grid) {                                                        // room for whichever grid the call may pick
+        size_t need = 0;
+        Opts t = o;
+        t.auto_grid = false;
+        for (t.grid_dims = 1; t.grid_dims <= 6 && t.grid_dims <= dim; ++t.grid_dims)
+            for (t.grid_bits = 2; t.grid_bits <= 8; ++t.grid_bits) {
+                if (!grid_within_budget(t.grid_dims, t.grid_bits, static_cast<double>(n_total) / n_events, n_events)) continue;
+                const size_t b = make_layout(n_total, n_events, GridChoice{t.grid_dims, t.grid_bits}, dim, o.order.on != 0).total;
+                if (b > need) need = b;
+            }
+        return need;
+    }
     return make_layout(n_total, n_events, choose_grid(o, n_total, n_events, dim), dim, o.order.on != 0).total;
 }
 
@@ -736,6 +769,28 @@ GridCost grid_cost(const double s[kDimMax][9], const unsigned char* order, int d
 
 struct GridTry { int g, bits, order; GridCost c; float measured_us; };
 
+// FRNN_GRID_AUTO: the model's best grid (default coordinate order) for this call's own rows
+int auto_grid(const float* points, int64_t n, int n_events, int dim, float r, cudaStream_t st, int* g_out, int* bits_out) {
+    SuggestOut so;
+    const int rc = run_suggest(points, n, dim, r, st, &so);
+    if (rc != FRNN_OK) return rc;
+    const double tot = so.sampled ? static_cast<double>(so.sampled) : 1.0;
+    double s[kDimMax][9];
+    for (int d = 0; d < kDimMax; ++d)
+        for (int b = 0; b <= 8; ++b) s[d][b] = (d < dim && b >= 2) ? pair_probability(so.hist[d], b, tot) : 1.0;
+    const unsigned char ident[8] = {0, 1, 2, 3, 4, 5, 6, 7};
+    const double n_event = static_cast<double>(n) / n_events;
+    double best = 0.0;
+    *g_out = 0;
+    for (int g = 1; g <= 6 && g <= dim; ++g)
+        for (int bits = 2; bits <= 8; ++bits) {
+            if (!grid_within_budget(g, bits, n_event, n_events)) continue;
+            const double us = grid_cost(s, ident, dim, g, bits, n_event, n_events).us;
+            if (*g_out == 0 || us < best) { best = us; *g_out = g; *bits_out = bits; }
+        }
+    return *g_out ? FRNN_OK : FRNN_ERR_UNSUPPORTED;
+}
+
 }  // namespace
 
 extern "C" {
@@ -838,15 +893,11 @@ int frnn_suggest_grid(const float* points, int64_t n, int n_events, int dim, flo
     }
     const int64_t n_first = n / n_events > 0 ? n / n_events : n;                  // rows of the sample event that is measured
     const double n_event = static_cast<double>(n) / n_events;
-    int ev_bits = 0;
-    while ((1ll << ev_bits) < n_events) ++ev_bits;
-    // table budget: 64 cells per point of an event (a finer table costs more to zero and scan than it saves), 2^26 in all
-    const double budget = fmin(fmax(65536.0, 64.0 * n_event), 67108864.0 / n_events);
     std::vector<GridTry> all;
     const bool same_order = memcmp(orders[0], orders[1], 8) == 0;
     for (int g = 1; g <= 6 && g <= dim; ++g)
         for (int bits = 2; bits <= 8; ++bits) {
-            if (g * bits + ev_bits > 30 || pow(2.0, g * bits) > budget) continue;
+            if (!grid_within_budget(g, bits, n_event, n_events)) continue;
             GridTry t{g, bits, 0, grid_cost(s, orders[0], dim, g, bits, n_event, n_events), 0.0f};
             if (!same_order) {                     // reorder only for a clear predicted gain: the default order is the fast path
                 const GridCost c1 = grid_cost(s, orders[1], dim, g, bits, n_event, n_events);

@@ -47,6 +47,7 @@ class FrnnGridReport(_c.Structure):
 
 
 FRNN_LAUNCH_DEFAULT, FRNN_LAUNCH_GRAPH, FRNN_LAUNCH_PLAIN = 0, 1, 2
+FRNN_GRID_AUTO = -1
 _OPT = _c.POINTER(FrnnOptions)
 _BUILD_ARGS = [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
                _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64,

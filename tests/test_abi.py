@@ -75,6 +75,10 @@ def test_options_struct_and_sizing():
     assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(order=[0, 1, 2])) == base   # the default order written out
     assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(9, 5)) == 0                # invalid options
     assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(order=[4, 4])) == 0
+    auto = frnn.frnn_options(frnn.FRNN_GRID_AUTO)
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, auto) >= max(
+        frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(g, b)) for g, b in ((4, 5), (3, 7), (2, 8), (5, 4)))   # room for any pick
+    assert frnn.frnn_workspace_bytes(120000, 1, 8, 256, frnn.frnn_options(-2)) == 0
     assert frnn.frnn_last_error_string() == ""
 
 

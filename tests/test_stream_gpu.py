@@ -387,6 +387,40 @@ def test_suggested_grid_on_wide_offset_and_fine_data(F, extent, r, offset):
         assert_same(host_result(res), exp, r, f"extent {extent} r {r} offset {offset} opt {'suggested' if o else 'default'}")
 
 
+def test_grid_chosen_per_call_from_the_event_itself(F):
+    """grid_dims = FRNN_GRID_AUTO: every call looks at its own rows first.  One workspace (sized for any grid the call may
+    pick), events whose extent / r differs by two orders of magnitude following each other: every result is the oracle's."""
+    n = 30000
+    opt = F.frnn_options(F.FRNN_GRID_AUTO)
+    ws = F.Workspace(n, 1, 32, n * 40, opt=opt)
+    assert ws.buf.numel() >= F.frnn_workspace_bytes(n, 1, 8, 32)
+    st = torch.cuda.Stream()
+    for extent, r, offset in ((2.0, 0.1, 0.0), (20.0, 0.1, 0.0), (2.0, 0.02, 0.0), (2.0, 0.3, 0.0), (2.0, 0.1, 1001.0), (2.0, 0.1, 0.0)):
+        x = spread_event(n, extent, 77, offset, sigma=0.3 * r)
+        exp = oracle.frnn(x, r, 32, oracle.CELLS)
+        res = F.frnn_build_ex(torch.from_numpy(x).cuda(), r, 32, ws=ws, stream=st, opt=opt)
+        st.synchronize()
+        res.check()
+        assert_same(host_result(res), exp, r, f"auto grid extent {extent} r {r} offset {offset}")
+    # batched, and tiny events
+    cfg = events.CONFIGS[0]
+    xb = np.ascontiguousarray(np.concatenate([events.make_event(cfg, 3)[:900], events.make_event(cfg, 4)[:17], events.make_event(cfg, 5)]))
+    offs = np.array([0, 900, 917, 917 + cfg.n], np.int64)
+    expb, eoffs = oracle.frnn_batched(xb, offs, cfg.r, 6)
+    resb = F.frnn_build_batched(torch.from_numpy(xb).cuda(), offs, cfg.r, 6, opt=opt)
+    torch.cuda.synchronize()
+    resb.check()
+    assert np.array_equal(resb.count.cpu().numpy(), eoffs)
+    s_, d_, q_ = (t.cpu().numpy() for t in resb.trimmed())
+    assert np.array_equal(s_, expb.src) and np.array_equal(d_, expb.dst) and np.array_equal(H.bits(q_), H.bits(expb.d2))
+    for m in (1, 2, 40):
+        xs = events.make_event(cfg, 6)[:m]
+        res = F.frnn_build_ex(torch.from_numpy(xs).cuda(), cfg.r, 4, opt=opt)
+        torch.cuda.synchronize()
+        res.check()
+        assert_same(host_result(res), oracle.frnn(xs, cfg.r, 4, oracle.BRUTE), cfg.r, f"auto grid n={m}")
+
+
 def test_suggest_grid_statistics_match_a_numpy_histogram(F):
     """The probabilities frnn_suggest_grid reports are those of the folded cell histogram of the points it sampled."""
     cfg = events.CONFIGS[1]
