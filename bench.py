@@ -462,7 +462,11 @@ def main() -> None:
                      "l2_bytes_per_launch": c.get("l2_bytes"), "traffic": c.get("dram_bytes"),
                      "dram_gbs": (c["dram_bytes"] / (dur_us * 1e-6) / 1e9) if c.get("dram_bytes") else None,
                      "dram_frac_of_hbm_peak": (c["dram_bytes"] / (dur_us * 1e-6) / 1e9 / peak) if c.get("dram_bytes") else None,
-                     "kernel_us": dur_us, "counters": "profiles/r02_counters.csv (ncu, one launch, cold cache)"}
+                     "kernel_us": dur_us, "counters": "profiles/r02_counters.csv (ncu, one launch, cold cache)",
+                     "ncu_cold": {"issue_active_pct": c.get("issue_active_pct"), "l1tex_pct_of_peak": c.get("l1tex_pct"), "l2_hit_pct": c.get("l2_hit_pct"),
+                                  "occupancy_pct": c.get("occupancy_pct"), "sm_active_over_elapsed": (c["sm_active_cycles"] / c["sm_elapsed_cycles"]) if c.get("sm_elapsed_cycles") else None,
+                                  "note": "the L1 data pipe (one wavefront per lane for the survivors' random 32-byte rows) is the busiest unit; neither it nor the "
+                                          "issue slots saturate: the kernel is a chain of ~27 dependent memory round trips per warp (profiles/r02_summary.md)"}}
         model = None
         if dur_us and model_bytes:
             ach = model_bytes / (dur_us * 1e-6) / 1e9
