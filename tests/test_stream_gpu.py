@@ -181,6 +181,20 @@ def test_config1_with_a_binding_k(F, k):
     assert_same(host_result(res), exp, cfg.r, f"cfg1 K={k}")
 
 
+@pytest.mark.parametrize("k", [2, 4])
+def test_config2_full_size_with_a_binding_k(F, k):
+    """The K-binding bench leg's workload at its own size: 120,000 points, a quarter of the rows over K = 4."""
+    cfg = events.CONFIGS[2]
+    x = events.make_event(cfg)
+    exp = oracle.frnn(x, cfg.r, k, oracle.CELLS)
+    assert (exp.uncapped > k).sum() > 20000
+    res = F.frnn_build_ex(torch.from_numpy(x).cuda(), cfg.r, k, edge_capacity=cfg.n * k, want_row_ptr=True)
+    torch.cuda.synchronize()
+    res.check()
+    assert_same(host_result(res), exp, cfg.r, f"cfg2 K={k}")
+    assert np.array_equal(np.diff(res.row_ptr.cpu().numpy()), np.minimum(exp.uncapped, k))
+
+
 @pytest.mark.parametrize("k", [1, 64, 200, 512, 600])
 def test_dense_rows_staged_and_beyond_staging(F, k):
     """Counts 99..699: up to 512 the row is collected once and selected by the bitonic network; beyond, the bisection
@@ -419,6 +433,25 @@ def test_grid_chosen_per_call_from_the_event_itself(F):
         torch.cuda.synchronize()
         res.check()
         assert_same(host_result(res), oracle.frnn(xs, cfg.r, 4, oracle.BRUTE), cfg.r, f"auto grid n={m}")
+
+
+def test_batched_config3_subset_with_suggested_and_odd_grids(F):
+    """Four of config 3's events in one batched call, through the measured suggestion and through two hand-picked grids."""
+    cfg = events.CONFIGS[2]
+    evs = [events.make_event(cfg, 100 + e)[: cfg.n - 1000 * e] for e in range(4)]
+    x = np.ascontiguousarray(np.concatenate(evs))
+    offs = np.concatenate([[0], np.cumsum([len(e) for e in evs])]).astype(np.int64)
+    exp, eoffs = oracle.frnn_batched(x, offs, cfg.r, cfg.k_max)
+    pts = torch.from_numpy(x).cuda()
+    sug, rep = F.frnn_suggest_grid(pts, cfg.r, n_events=4, measure=True)
+    assert rep.n_tried >= 1
+    for opt in (sug, F.frnn_options(3, 6), F.frnn_options(5, 4, [7, 6, 5, 4, 3])):
+        res = F.frnn_build_batched(pts, offs, cfg.r, cfg.k_max, edge_capacity=len(x) * 4, opt=opt)
+        torch.cuda.synchronize()
+        res.check()
+        assert np.array_equal(res.count.cpu().numpy(), eoffs)
+        s_, d_, q_ = (t.cpu().numpy() for t in res.trimmed())
+        assert np.array_equal(s_, exp.src) and np.array_equal(d_, exp.dst) and np.array_equal(H.bits(q_), H.bits(exp.d2))
 
 
 def test_suggest_grid_statistics_match_a_numpy_histogram(F):
