@@ -1046,27 +1046,56 @@ __device__ __forceinline__ void warp_sort_keys(unsigned long long* k, int p2, in
 
 // Warp top-K on staged keys (north_star (3): per-query K-cap selection on (d2, index) with index tie-break): the k
 // smallest of the n distinct 64-bit keys key[0..n) (d2 bits << 32 | j, d2 bits <= hi_max) are moved to key[0..k), in no
-// particular order, and the k-th smallest key is returned.  Bisection on the bit pattern of d2 (every step counts, with
-// one pass over the staged keys and a warp reduction, how many lie at or below the probe), then -- only if several keys
-// share the k-th d2 and not all of them are wanted -- on j among those; then a stable in-place compaction.  n <= kStage,
-// 1 <= k < n.  All lanes must call it; the caller has made the staged keys visible (__syncwarp).
-__device__ __forceinline__ unsigned long long warp_select_keys(unsigned long long* key, uint32_t n, uint32_t k, uint32_t hi_max,
+// particular order, and the k-th smallest key is returned.  Radix select on the bit pattern of d2 (four passes of one byte,
+// each a shared-memory histogram over the staged keys that match the bytes fixed so far), then -- only if several keys
+// share the k-th d2 and not all of them are wanted -- a bisection on j among those; then a stable in-place compaction.
+// n <= kStage, 1 <= k < n; hist: 256 words of the warp.  All lanes must call it; the staged keys are visible (__syncwarp).
+__device__ __forceinline__ unsigned long long warp_select_keys(unsigned long long* key, uint32_t n, uint32_t k, uint32_t* hist,
                                                                int lane, uint32_t lt_mask) {
     const uint32_t* w = reinterpret_cast<const uint32_t*>(key);       // w[2t] = j, w[2t+1] = d2 bits (little endian)
-    uint32_t lo = 0, hi = hi_max;
-    while (lo < hi) {
-        const uint32_t mid = lo + ((hi - lo) >> 1);
-        uint32_t c = 0;
-        for (uint32_t t = lane; t < n; t += 32) c += w[2 * t + 1] <= mid;
-        c = __reduce_add_sync(kFull, c);
-        if (c >= k) hi = mid; else lo = mid + 1;
+    // the k-th smallest d2 by a radix select, one byte per pass from the top: histogram (256 bins of the warp, shared memory)
+    // of that byte over the keys that match the bytes fixed so far, then the bin that holds the kk-th of them
+    uint32_t prefix = 0, fixed = 0, kk = k, c_eq = 0;
+#pragma unroll 1
+    for (int shift = 24; shift >= 0; shift -= 8) {
+#pragma unroll
+        for (int b = 0; b < 8; ++b) hist[lane * 8 + b] = 0u;
+        __syncwarp();
+        for (uint32_t t = lane; t < n; t += 32) {
+            const uint32_t d = w[2 * t + 1];
+            if ((d & fixed) == prefix) atomicAdd(&hist[(d >> shift) & 255u], 1u);
+        }
+        __syncwarp();
+        uint32_t loc[8], sum = 0;
+#pragma unroll
+        for (int b = 0; b < 8; ++b) { loc[b] = hist[lane * 8 + b]; sum += loc[b]; }
+        uint32_t incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t x = __shfl_up_sync(kFull, incl, o);
+            if (lane >= o) incl += x;
+        }
+        const uint32_t excl = incl - sum;
+        const bool mine = excl < kk && kk <= incl;                    // exactly one lane holds the kk-th key
+        uint32_t bin = 0, before = excl, inbin = 0;
+        if (mine) {
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                if (before < kk && kk <= before + loc[b]) { bin = static_cast<uint32_t>(lane * 8 + b); inbin = loc[b]; break; }
+                before += loc[b];
+            }
+        }
+        const int src = __ffs(__ballot_sync(kFull, mine)) - 1;
+        bin = __shfl_sync(kFull, bin, src);
+        before = __shfl_sync(kFull, before, src);
+        c_eq = __shfl_sync(kFull, inbin, src);
+        prefix |= bin << shift;
+        fixed |= 255u << shift;
+        kk -= before;
+        __syncwarp();
     }
-    const uint32_t dk = lo;                                           // the k-th smallest d2
-    uint32_t c_lt = 0, c_eq = 0;
-    for (uint32_t t = lane; t < n; t += 32) { const uint32_t d = w[2 * t + 1]; c_lt += d < dk; c_eq += d == dk; }
-    c_lt = __reduce_add_sync(kFull, c_lt);
-    c_eq = __reduce_add_sync(kFull, c_eq);
-    const uint32_t need = k - c_lt;                                   // how many of the keys with d2 == dk are wanted (>= 1)
+    const uint32_t dk = prefix;                                       // the k-th smallest d2; c_eq keys share it
+    const uint32_t need = kk;                                         // how many of those are wanted (>= 1)
     uint32_t jk = 0x7fffffffu;
     if (need < c_eq) {                                                // ties at the k-th d2: the smallest indices win
         uint32_t jlo = 0, jhi = 0x7fffffffu;
@@ -1129,7 +1158,7 @@ struct EmitArgs {
 template <int G, bool INTERIOR>
 __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int64_t row_rp, int64_t row_ev, uint32_t row_cnt,
                                           uint32_t cell, const float4& qa, const float4& qb, int* s_delta,
-                                          unsigned long long* stage, int lane, int lane_delta, uint32_t lt_mask) {
+                                          unsigned long long* stage, uint32_t* hist, int lane, int lane_delta, uint32_t lt_mask) {
     const float inf = __int_as_float(0x7f800000);
     const bool hi = a.dim > kDim;                         // coordinates 8..15 exist: the chain goes on over them
     float4 qc = make_float4(0.f, 0.f, 0.f, 0.f), qd = qc;
@@ -1191,14 +1220,14 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
             if (fill > static_cast<uint32_t>(kStage - 32) && fill > a.k_max) {       // (K <= kStage / 2 here, or the row would fit)
                 __syncwarp();
                 thr = warp_select_keys(stage, fill < static_cast<uint32_t>(kStage) ? fill : static_cast<uint32_t>(kStage), a.k_max,
-                                       __float_as_uint(a.r2), lane, lt_mask);
+                                       hist, lane, lt_mask);
                 fill = a.k_max;
             }
         });
         __syncwarp();
         if (fill > static_cast<uint32_t>(kStage)) fill = kStage;                     // (cannot happen: see the prune condition)
         if (fill > a.k_max) {                             // S8: the K smallest keys
-            warp_select_keys(stage, fill, a.k_max, __float_as_uint(a.r2), lane, lt_mask);
+            warp_select_keys(stage, fill, a.k_max, hist, lane, lt_mask);
             fill = a.k_max;
         }
         const uint32_t len = fill;
@@ -1278,6 +1307,7 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     __shared__ uint32_t s_kept[kEmitThreads];              // medium rows: bit h set = stored hit h is among the K nearest
     __shared__ uint32_t s_mwarp[kEmitThreads / 32];
     __shared__ unsigned long long s_stage[kEmitThreads / 32][kStage];   // big rows: per-warp staging of (d2, j) keys
+    __shared__ uint32_t s_hist[kEmitThreads / 32][256];                 // big rows: per-warp histogram of the radix select
     __shared__ unsigned int s_done;                        // timeline only: threads of the block that have finished
     if (threadIdx.x == 0) s_done = 0u;                     // (made visible by the barriers below)
     stamp_begin(a.stamps, 4);
@@ -1472,8 +1502,8 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
                 const uint32_t cd = (cell >> (d * a.bits)) & mask;
                 interior = interior && cd != 0u && cd != mask;
             }
-            if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], lane, lane_delta, lt_mask);
-            else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], lane, lane_delta, lt_mask);
+            if (interior) emit_big_row<G, true>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], s_hist[warp], lane, lane_delta, lt_mask);
+            else          emit_big_row<G, false>(a, row, row_rp, row_ev, row_cnt, cell, qa, qb, s_delta[warp], s_stage[warp], s_hist[warp], lane, lane_delta, lt_mask);
         }
     }
     stamp_end_last(a.stamps, 4, &s_done);
