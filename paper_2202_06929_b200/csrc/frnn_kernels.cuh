@@ -994,6 +994,8 @@ __global__ void __launch_bounds__(kPrefixThreads) tile_prefix_kernel(PrefixArgs 
 //                                in place by a bitonic network in global memory
 // ------------------------------------------------------------------------------------------------
 constexpr int kStage = 512;            // staging entries per warp for recomputed rows (K <= 512: 16 keys per lane)
+constexpr int kRankMax = 192;          // up to this many kept hits are ordered by rank counting, more by the bitonic network
+template <int V> struct IntTag { static constexpr int value = V; };
 
 __device__ __forceinline__ void cmp_swap(int32_t* dst, float* d2, int64_t lo, int64_t hi) {
     const int32_t x = dst[lo], y = dst[hi];
@@ -1231,7 +1233,43 @@ __device__ __forceinline__ void emit_big_row(const EmitArgs& a, int64_t row, int
             fill = a.k_max;
         }
         const uint32_t len = fill;
-        // ---- order the kept hits by dst: keys (j << 32 | d2 bits), bitonic sort
+        // ---- order the kept hits by dst.  Up to kRankMax of them: every lane ranks its (at most kRankMax / 32) hits by counting
+        // the kept hits with a smaller j -- one broadcast shared load per kept hit, no dependent chain -- and stores each at
+        // its rank (the stores of a row fall into one window of a few hundred bytes).  More: keys (j << 32 | d2 bits) through
+        // the bitonic network, coalesced stores.
+        if (len <= static_cast<uint32_t>(kRankMax)) {
+            const uint32_t* w = reinterpret_cast<const uint32_t*>(stage);   // w[2t] = j, w[2t+1] = d2 bits
+            auto rank_and_store = [&](auto e_tag) {
+                constexpr int E = decltype(e_tag)::value;                   // kept hits per lane
+                uint32_t myj[E], rank[E];
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const uint32_t t = lane + 32u * e;
+                    myj[e] = t < len ? w[2 * t] : 0xffffffffu;
+                    rank[e] = 0u;
+                }
+#pragma unroll 4
+                for (uint32_t u = 0; u < len; ++u) {
+                    const uint32_t ju = w[2 * u];
+#pragma unroll
+                    for (int e = 0; e < E; ++e) rank[e] += ju < myj[e];
+                }
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const uint32_t t = lane + 32u * e;
+                    const int64_t pos = row_rp + rank[e];
+                    if (t < len && pos < a.capacity) {
+                        a.out_src[pos] = src;
+                        a.out_dst[pos] = static_cast<int32_t>(myj[e]) - static_cast<int32_t>(row_ev);
+                        a.out_d2[pos] = __uint_as_float(w[2 * t + 1]);
+                    }
+                }
+            };
+            if (len <= 64u) rank_and_store(IntTag<2>{});
+            else            rank_and_store(IntTag<kRankMax / 32>{});
+            __syncwarp();
+            return;
+        }
         int p2 = 2;
         while (static_cast<uint32_t>(p2) < len) p2 <<= 1;
         for (int t = lane; t < p2; t += 32) {
