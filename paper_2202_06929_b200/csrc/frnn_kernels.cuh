@@ -845,7 +845,10 @@ struct DenseArgs {
 // paid once per kDenseQ pairs -- 16 kDenseQ FP32 instructions per 2 loads instead of 16.  Block (I, J): queries
 // [I * kDenseQ * 128, +kDenseQ * 128) x candidates [J * 128, +128); blocks entirely below the diagonal leave at once, blocks
 // on it test j > i per pair.
-template <bool HI> struct DenseCfg { static constexpr int Q = HI ? 2 : 4; };
+#ifndef FRNN_DENSE_Q
+#define FRNN_DENSE_Q 4
+#endif
+template <bool HI> struct DenseCfg { static constexpr int Q = HI ? 2 : FRNN_DENSE_Q; };
 
 // a hit of the brute-force search (rare: kept out of line so that the pair loop stays tight)
 __device__ __noinline__ void dense_hit(const DenseArgs& a, unsigned long long* my_tile_deg, int32_t row, int32_t cj, float d2) {
@@ -858,25 +861,44 @@ __device__ __noinline__ void dense_hit(const DenseArgs& a, unsigned long long* m
     if (p1 < a.k_max) atomicAdd(&my_tile_deg[cj / kEmitThreads], 1ull);
 }
 
+// kDenseStep candidate rows per step: Q x kDenseStep chains run, ONE predicate collects "some pair is within r" (an FSETP
+// per pair that ORs into it, no branch), and only a step that has a hit goes through its pairs again to commit them --
+// a branch per step instead of one per pair (hits are rare: 2.3e-5 of the pairs of a tracking event).
+#ifndef FRNN_DENSE_STEP
+#define FRNN_DENSE_STEP 4
+#endif
+constexpr int kDenseStep = FRNN_DENSE_STEP;
 template <bool HI, bool DIAG, int Q>
 __device__ __forceinline__ void dense_pairs(const DenseArgs& a, const float4 (*s_c)[HI ? 4 : 2], const float4* qa, const float4* qb,
                                             const float4* qc, const float4* qd, const int* qrel, int64_t q_lo, int64_t c_lo,
                                             unsigned long long* my_tile_deg, int tid) {
-#pragma unroll 4
-    for (int k = 0; k < kDenseTile; ++k) {
-        const float4 ka = s_c[k][0], kb = s_c[k][1];
-        float d2[Q];
+#pragma unroll 1
+    for (int k0 = 0; k0 < kDenseTile; k0 += kDenseStep) {
+        float d2[kDenseStep][Q];
 #pragma unroll
-        for (int q = 0; q < Q; ++q) d2[q] = d2_pinned(qa[q], qb[q], ka, kb);
-        if (HI) {
-            const float4 kc = s_c[k][2], kd = s_c[k][3];
+        for (int s = 0; s < kDenseStep; ++s) {
+            const float4 ka = s_c[k0 + s][0], kb = s_c[k0 + s][1];
 #pragma unroll
-            for (int q = 0; q < Q; ++q) d2[q] = d2_continue(d2[q], qc[q], qd[q], kc, kd);
+            for (int q = 0; q < Q; ++q) d2[s][q] = d2_pinned(qa[q], qb[q], ka, kb);
+            if (HI) {
+                const float4 kc = s_c[k0 + s][2], kd = s_c[k0 + s][3];
+#pragma unroll
+                for (int q = 0; q < Q; ++q) d2[s][q] = d2_continue(d2[s][q], qc[q], qd[q], kc, kd);
+            }
         }
+        bool any = false;
 #pragma unroll
-        for (int q = 0; q < Q; ++q)
-            if (d2[q] <= a.r2 && (!DIAG || k > qrel[q]))
-                dense_hit(a, my_tile_deg, static_cast<int32_t>(q_lo + q * kDenseTile + tid), static_cast<int32_t>(c_lo + k), d2[q]);
+        for (int s = 0; s < kDenseStep; ++s)
+#pragma unroll
+            for (int q = 0; q < Q; ++q) any = any || d2[s][q] <= a.r2;
+        if (any) {
+#pragma unroll
+            for (int s = 0; s < kDenseStep; ++s)
+#pragma unroll
+                for (int q = 0; q < Q; ++q)
+                    if (d2[s][q] <= a.r2 && (!DIAG || k0 + s > qrel[q]))
+                        dense_hit(a, my_tile_deg, static_cast<int32_t>(q_lo + q * kDenseTile + tid), static_cast<int32_t>(c_lo + k0 + s), d2[s][q]);
+        }
     }
 }
 
