@@ -383,28 +383,37 @@ def main() -> None:
     # dependent graph nodes overlaps the other event's work.  Reported beside the headline, which stays one stream.
     two_streams = None
     if "two_streams" in legs and args.two_stream_steps > 0:
-        stream_b = torch.cuda.Stream(dev)
-        scratch_b = torch.empty_like(shared)
-        args_b = [a[:12] + (C.c_void_p(scratch_b.data_ptr()), scratch_b.numel(), C.c_void_p(stream_b.cuda_stream)) for a in call_args]
-        for i in range(len(call_args)):                       # build the graph of the second workspace
-            assert build_ex(*args_b[i]) == 0
-        torch.cuda.synchronize()
-        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        ea.record(stream)
-        stream_b.wait_event(ea)
-        for i in range(args.two_stream_steps):
-            k = i % len(call_args)
-            st = build_ex(*(call_args[k] if i % 2 == 0 else args_b[k]))     # outputs k are only touched by step i
-            assert st == 0
-        done_b = torch.cuda.Event()
-        done_b.record(stream_b)
-        stream.wait_event(done_b)
-        eb.record(stream)
-        torch.cuda.synchronize()
-        ms2 = ea.elapsed_time(eb) / args.two_stream_steps
+        def in_flight(n_streams: int) -> float:
+            """ms per event with `n_streams` events in flight: events go round-robin to n_streams streams, each with its own scratch"""
+            extra = [torch.cuda.Stream(dev) for _ in range(n_streams - 1)]
+            scratch = [torch.empty_like(shared) for _ in extra]
+            per_stream = [call_args] + [[a[:12] + (C.c_void_p(sc.data_ptr()), sc.numel(), C.c_void_p(st.cuda_stream)) for a in call_args]
+                                        for st, sc in zip(extra, scratch)]
+            for lst in per_stream[1:]:                            # build the graphs of the other workspaces
+                for i in range(min(len(lst), 4)):
+                    assert build_ex(*lst[i]) == 0
+            torch.cuda.synchronize()
+            ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ea.record(stream)
+            for st in extra:
+                st.wait_event(ea)
+            for i in range(args.two_stream_steps):
+                st = build_ex(*per_stream[i % n_streams][i % len(call_args)])     # outputs i % pool are only touched by step i
+                assert st == 0
+            for st in extra:
+                done = torch.cuda.Event()
+                done.record(st)
+                stream.wait_event(done)
+            eb.record(stream)
+            torch.cuda.synchronize()
+            return ea.elapsed_time(eb) / args.two_stream_steps
+
+        ms2 = in_flight(2)
+        ms4 = in_flight(4)
         two_streams = {"ms_per_event": ms2, "edges_per_s": e_mean_all / (ms2 * 1e-3), "steps": args.two_stream_steps,
-                       "note": "same call, events alternate between two streams with their own scratch workspace"}
-        del scratch_b
+                       "four_streams": {"ms_per_event": ms4, "edges_per_s": e_mean_all / (ms4 * 1e-3)},
+                       "note": "same call, events go round-robin to 2 (4) streams with their own scratch workspace: the fixed latency of "
+                               "one event's six dependent graph nodes overlaps the other events' work"}
 
     # per-phase device times (separate loop: event records between kernels perturb the main timing)
     phases_us = None
