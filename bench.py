@@ -143,7 +143,7 @@ class ClockSampler(threading.Thread):
             mask |= s[2]
         return {"sm_mhz": float(np.median([s[1] for s in sel])), "sm_max_mhz": self.max_mhz,
                 "reasons": sorted(n for b, n in REASONS.items() if mask & b), "samples": len(sel),
-                "how": "NVML, one reading right before and right after the timed loop (GPU busy) + every 5 ms in between"}
+                "how": "NVML: one reading while the warm-up steps are in flight, one right after the last timed step was submitted (GPU busy at both), and every 5 ms in between"}
 
 
 def oracle_sample_run(n_events: int, threads: int = 0):
@@ -301,19 +301,18 @@ def main() -> None:
     sampler = ClockSampler(uuid, rank.local_rank)
     sampler.start()
     with torch.cuda.stream(stream):
+        t_clk0 = time.perf_counter()
         for i in range(args.warmup):
             step(i)
+        sampler.sample_now()                          # clocks under load, taken OUTSIDE the timed region: the warm-up steps are in flight
         stream.synchronize()
         D.barrier(rank)
         torch.cuda.synchronize()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
         ev0.record(stream)
-        for i in range(min(args.steps, 8)):
-            step(i)
-        sampler.sample_now()                          # the GPU is busy with the first steps
-        for i in range(min(args.steps, 8), args.steps):
-            step(i)
+        for i in range(args.steps):                   # nothing but the calls between the two events: a synchronous NVML reading
+            step(i)                                   # inside this loop would leave the GPU idle for longer than a 20-step run lasts
         ev1.record(stream)
         sampler.sample_now()                          # the last steps are still in flight
         torch.cuda.synchronize()
@@ -326,7 +325,7 @@ def main() -> None:
     total_edges = D.reduce_sum(my_edges, rank)
     value = total_edges / (ms * 1e-3)
     ms_per_step = ms / args.steps
-    clocks = sampler.summary(t0, t1)
+    clocks = sampler.summary(t_clk0, t1)
     e_mean_all = float(np.mean(edges_per_event))
     peak, sm_max_mhz, peak_src = measured_peaks()
     sm_mhz = clocks.get("sm_mhz") or sm_max_mhz
