@@ -245,6 +245,43 @@ int frnn_build_dense_ex(const float* points, int64_t n, int dim, float r, int k_
                         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * frnn_build_static -- frnn_build_ex for callers that must not (or cannot) allocate device memory.
+ *
+ * Who this is for.  Track finding runs inside larger programs that often forbid allocation on the path where an
+ * event is processed: an online / trigger process that hands all of the GPU's memory to its framework's arena when
+ * it is configured, so that a later cudaMalloc fails or breaks the memory budget; a latency-bound event loop, where
+ * cudaMalloc and cudaFree are ruled out because they stall the whole device for an unpredictable time; a plug-in
+ * that runs under somebody else's allocator and has no way to ask it for scratch.  Such a caller can still hand
+ * over its input and output arrays, but has nowhere to take a workspace from.
+ *
+ * What it does.  Same operation, same arguments, same result (bit for bit) and same error behaviour as
+ * frnn_build_ex (section 2, section 3.4; S1..S10 of SURVEY.md section 8(a)), minus the two
+ * workspace arguments: the scratch is a fixed array of frnn_static_scratch_bytes() = 3 MiB that is part of the
+ * library's device image.  Every GPU on which the library's code is loaded holds those 3 MiB until the process ends,
+ * used or not -- hence the small limit:
+ *     n <= FRNN_STATIC_MAX_ROWS (8192 rows), any dim 1..16.
+ * A larger n returns FRNN_ERR_UNSUPPORTED, enqueues nothing, touches no output, and leaves a sentence saying so in
+ * frnn_last_error_string().  The entry point calls no cudaMalloc / cudaFree and nothing that allocates device memory:
+ * it uses the automatic grid and the default coordinate order (frnn_set_grid / frnn_set_bin_order do not apply, the
+ * array is sized for that layout) and enqueues its memset and kernels one by one on cuda_stream (no CUDA-graph
+ * executable is built; frnn_set_graph_mode does not apply).  Asynchronous like frnn_build_ex.
+ *
+ * Rules that come with a shared array:
+ *   - First call on a device: it looks up the array's device address (once per device, for the device that is
+ *     current at the call) before enqueuing.  Make that first call at set-up time, outside any stream capture.
+ *   - All calls on one device use the SAME array.  The call clears what it needs cleared itself, so leftovers of an
+ *     earlier call are harmless; but two calls whose work overlaps on the GPU (different streams without an
+ *     ordering between them, or two host threads) overwrite each other's scratch and produce garbage.  Keep the
+ *     calls of a device on one stream, or order them with events.
+ *   - Devices are independent: each has its own copy of the array.
+ */
+#define FRNN_STATIC_MAX_ROWS 8192
+size_t frnn_static_scratch_bytes(void);
+int frnn_build_static(const float* points, int64_t n, int dim, float r, int k_max,
+                      int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                      int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr, void* cuda_stream);
+
+/*
  * Batched events (BASELINE.json config 3): n_events independent events concatenated in `points`;
  * event e owns rows [event_offsets[e], event_offsets[e+1]) (HOST int64[n_events+1], ascending,
  * event_offsets[0] == 0).  No cross-event edges.  src/dst are LOCAL to the event.  Edges of event

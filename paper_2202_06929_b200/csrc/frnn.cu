@@ -793,6 +793,50 @@ int auto_grid(const float* points, int64_t n, int n_events, int dim, float r, cu
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------
+// Scratch of frnn_build_static (include/frnn.h): the workspace of one small single-event build, reserved inside the
+// library image itself so that the entry point never has to ask the CUDA runtime for device memory.  Every device
+// that loads the library carries its own copy of these bytes from the moment the module is loaded until the process
+// exits, which is why the limit is kept small (FRNN_STATIC_MAX_ROWS rows).
+// The NAME below means two different things.  In device code it is the array.  In host code it is only a handle the
+// runtime knows the array by -- it is NOT a device address, and a kernel handed `g_static_scratch` from the host
+// would read and write the wrong memory.  Host code therefore asks the runtime for the real address, once per
+// device and with that device current (static_scratch_for_current_device), and passes that to the kernels.
+// ------------------------------------------------------------------------------------------------
+constexpr size_t kStaticScratchBytes = 3u << 20;          // 3 MiB: the 8192-row, dim 9..16 layout needs 2,923,520 bytes
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+void* g_static_ptr[kStaticMaxDevices] = {};                // device address of g_static_scratch, per device ordinal
+std::mutex g_static_mutex;
+
+// Device address of the current device's copy of g_static_scratch.  The first call on a device asks the runtime for it
+// (that may load the module: it must not happen while a stream is being captured); later calls read the cached value.
+int static_scratch_for_current_device(void** out) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) {
+        snprintf(t_error, sizeof(t_error), "frnn_build_static: device ordinal %d outside 0..%d", dev, kStaticMaxDevices - 1);
+        return FRNN_ERR_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        CK(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || reinterpret_cast<uintptr_t>(p) % kAlign) {
+            snprintf(t_error, sizeof(t_error), "frnn_build_static: cudaGetSymbolAddress returned an unusable address %p", p);
+            return FRNN_ERR_CUDA;
+        }
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return FRNN_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 int frnn_version(void) { return 400; }   // 0.4.0
@@ -1028,6 +1072,36 @@ int frnn_build_dense_ex(const float* points, int64_t n, int dim, float r, int k_
                         void* workspace, size_t workspace_bytes, void* cuda_stream) {
     return build_single(default_opts(), true, points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, out_status,
                         out_row_ptr, workspace, workspace_bytes, cuda_stream);
+}
+
+// The build of frnn_build_ex for callers that cannot allocate device memory (see include/frnn.h): same kernels, same
+// result, but the workspace is g_static_scratch and the kernels are enqueued one by one (building a graph executable
+// would allocate).  Nothing here, and nothing it calls, uses cudaMalloc, cudaFree or a library routine that allocates
+// device memory.  The memset at the head of the enqueued work zeroes the part of the scratch that must start at zero
+// (cell table, tile totals, counters, per-row counts), so what the previous call left behind does no harm.
+size_t frnn_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+int frnn_build_static(const float* points, int64_t n, int dim, float r, int k_max,
+                      int32_t* out_src, int32_t* out_dst, float* out_d2, int64_t edge_capacity,
+                      int64_t* out_count, int32_t* out_status, int64_t* out_row_ptr, void* cuda_stream) {
+    if (n > FRNN_STATIC_MAX_ROWS) {
+        snprintf(t_error, sizeof(t_error), "frnn_build_static: n = %lld exceeds FRNN_STATIC_MAX_ROWS = %d (use frnn_build_ex with a caller-owned workspace)",
+                 static_cast<long long>(n), FRNN_STATIC_MAX_ROWS);
+        return FRNN_ERR_UNSUPPORTED;
+    }
+    Opts o;                                    // the automatic grid and the default order whatever the process-wide setters say:
+    o.use_graph = false;                       // the scratch is sized for exactly that layout; plain launches (no graph objects)
+    if (n > 0 && dim >= 1 && dim <= kDimMax && k_max >= 1 &&
+        workspace_bytes_for(o, n, 1, dim, k_max) > kStaticScratchBytes) {          // cannot happen within the row limit; kept as a guard
+        snprintf(t_error, sizeof(t_error), "frnn_build_static: the layout of n = %lld rows needs more than the %zu scratch bytes",
+                 static_cast<long long>(n), kStaticScratchBytes);
+        return FRNN_ERR_UNSUPPORTED;
+    }
+    void* scratch = nullptr;
+    const int rc = static_scratch_for_current_device(&scratch);
+    if (rc != FRNN_OK) return rc;
+    return build_single(o, false, points, n, dim, r, k_max, out_src, out_dst, out_d2, edge_capacity, out_count, out_status,
+                        out_row_ptr, scratch, kStaticScratchBytes, cuda_stream);
 }
 
 int frnn_build_batched(const float* points, const int64_t* event_offsets, int n_events, int dim, float r, int k_max,

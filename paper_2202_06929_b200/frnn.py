@@ -75,6 +75,8 @@ _SIGNATURES = {
                               _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.POINTER(_c.c_int64)]),
     "frnn_build_ex": (_c.c_int, _BUILD_ARGS),
     "frnn_build_dense_ex": (_c.c_int, _BUILD_ARGS),
+    "frnn_static_scratch_bytes": (_c.c_size_t, []),
+    "frnn_build_static": (_c.c_int, _BUILD_ARGS[:12] + [_c.c_void_p]),
     "frnn_build_batched": (_c.c_int, _BATCHED_ARGS),
     "frnn_build_host": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_float, _c.c_int,
                                    _c.c_void_p, _c.c_void_p, _c.c_void_p, _c.c_int64, _c.POINTER(_c.c_int64)]),
@@ -318,6 +320,37 @@ def frnn_build_ex(points: torch.Tensor, r: float, k_max: int, edge_capacity: int
         st = getattr(lib(), _entry)(*args)
     _check(st, _entry)
     return EdgeList(ws.src, ws.dst, ws.d2, ws.count, ws.status, ws.row_ptr)
+
+
+FRNN_STATIC_MAX_ROWS = 8192
+
+
+def frnn_static_scratch_bytes() -> int:
+    """Size of the library's built-in scratch array (held by every GPU that loads the library)."""
+    return int(lib().frnn_static_scratch_bytes())
+
+
+def frnn_build_static(points: torch.Tensor, r: float, k_max: int, out_src: torch.Tensor, out_dst: torch.Tensor,
+                      out_d2: torch.Tensor, out_count: torch.Tensor, out_status: torch.Tensor,
+                      out_row_ptr: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None) -> EdgeList:
+    """``frnn_build_static`` of include/frnn.h: the single-event build for callers that cannot allocate device
+    memory on their event path (all memory handed to a framework arena at configure time, a latency-bound loop where
+    ``cudaMalloc`` would stall the device, a plug-in under a foreign allocator).  The scratch is a 3 MiB array inside
+    the library, so ``points`` may have at most ``FRNN_STATIC_MAX_ROWS`` rows; the caller passes every output
+    (``out_src/out_dst/out_d2``: equally long device arrays = the edge capacity; ``out_count`` int64[1];
+    ``out_status`` int32[1]; optional ``out_row_ptr`` int64[n+1]) and this wrapper allocates no tensor either.
+    All calls on a device share the one scratch array: keep them ordered on the GPU (one stream, or events);
+    make the first call on a device outside any stream capture.  Asynchronous on ``stream``."""
+    _require_cuda(points)
+    n, dim = points.shape
+    cap = min(out_src.numel(), out_dst.numel(), out_d2.numel())
+    stream = stream or torch.cuda.current_stream(points.device)
+    st = lib().frnn_build_static(_ptr(points), n, dim, float(r), int(k_max), _ptr(out_src), _ptr(out_dst), _ptr(out_d2), int(cap),
+                                 _ptr(out_count), _ptr(out_status), _ptr(out_row_ptr), _c.c_void_p(stream.cuda_stream))
+    if st == FRNN_ERR_UNSUPPORTED and n > FRNN_STATIC_MAX_ROWS:
+        raise FrnnError(st, f"frnn_build_static [{frnn_last_error_string()}]")
+    _check(st, "frnn_build_static")
+    return EdgeList(out_src, out_dst, out_d2, out_count, out_status, out_row_ptr)
 
 
 def frnn_build_opt(opt: FrnnOptions | None, points: torch.Tensor, r: float, k_max: int, **kw) -> EdgeList:
