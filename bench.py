@@ -7,10 +7,14 @@ stream.  Steps rotate over a pool of distinct events and distinct output buffers
 exceeds the 126 MB L2, so every step reads its input cold from HBM and every call differs from the previous one
 in its pointers (the library rewrites the graph's node parameters every step: nothing is a replay of an identical call).
 
-Prints ONE JSON line (rank 0).  Keys beyond the base contract:
-  roofline / roofline_issue   the dominant kernel against the bound that actually binds it: warp instructions per
-                launch (committed ncu counters, profiles/r02_counters.csv) / its in-graph duration vs the issue peak
-                148 SMs x 4 schedulers x measured SM clock ("bound": "alu")
+Prints ONE compact JSON line (rank 0) as the last thing on stdout: the contract keys only (metric, value, config,
+roofline, cpu_baseline, e2e, clocks, gpu_launches; under 4 KB -- the round-2 line carried every leg, grew to 21.6 KB
+and the driver could not read it).  The FULL report goes to gpurun_out/bench_full.json and, as one line, to stderr:
+  roofline      the dominant kernel against the bound that actually binds it: warp instructions per launch (committed
+                ncu counters, profiles/r0N_counters.csv; `counters_stale` says whether they belong to the kernel source
+                in the tree) / its in-graph duration vs the issue peak 148 SMs x 4 schedulers x measured SM clock
+                ("bound": "alu"); `traffic` = measured DRAM bytes of that launch, `dram_frac_of_hbm_peak` their rate
+                against MEASURED_PEAKS.json; `model_frac_hbm_equivalent` = north_star's byte model (not physical)
   roofline_model  north_star's figure for the same kernel: candidate-row bytes of the grid run / duration vs the measured
                 HBM peak.  These bytes are served by L2/L1: an HBM-EQUIVALENT rate, not a physical fraction (can exceed 1)
   path_roofline north_star's whole-path figure: (candidate rows * 32 B + 12 B * edges) / ms_per_event
@@ -21,7 +25,7 @@ Prints ONE JSON line (rank 0).  Keys beyond the base contract:
   cpu_baseline  the oracle (cell-list mode) on this box's host cores on a bounded sample, all cores and one thread;
                 brute-force mode once on configs 0-2
   e2e           the same metric through frnn_host_pipeline_*: pinned host buffers, H2D + D2H inside; a bare-copy floor
-                (the same bytes, no build) beside it; one event checked against the oracle
+                (the same bytes, no build) beside it; events of the timed loop checked against the oracle
 `--impl reference` times the oracle alone (rank 0 only) on the same metric/config.
 `--legs a,b,..` restricts the run to some legs (for ncu captures): headline is always run.
 """
@@ -64,16 +68,103 @@ def measured_peaks():
         return FALLBACK_HBM_GBS, 1965.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_counters():
-    """profiles/r02_counters.csv: per (workload, kernel) the ncu figures of ONE launch (see profiles/r02_counters.md)."""
-    out = {}
+KERNELS_SOURCE = os.path.join(ROOT, "paper_2202_06929_b200", "csrc", "frnn_kernels.cuh")
+COUNTER_FILES = ("r03_counters.csv", "r02_counters.csv")      # the newest capture that is committed wins
+FULL_REPORT = os.path.join("gpurun_out", "bench_full.json")   # every leg in full; the stdout line holds the contract keys only
+COMPACT_LIMIT = 4096                                           # bytes; tests/test_bench_line.py holds the line to it
+
+
+def blob_hash(path: str) -> str | None:
+    """What `git hash-object <path>` prints (sha1 of "blob <size>\\0" + content); None if the file is absent."""
+    import hashlib
     try:
-        with open(os.path.join(ROOT, "profiles", "r02_counters.csv")) as f:
-            for row in csv.DictReader(f):
-                out[(row["workload"], row["kernel"])] = {k: float(v) for k, v in row.items() if k not in ("workload", "kernel", "profile")}
-    except Exception:
-        pass
-    return out
+        data = open(path, "rb").read()
+    except OSError:
+        return None
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def ncu_counters():
+    """profiles/r0N_counters.csv: per (workload, kernel) the ncu figures of ONE launch (see the .md beside it).
+    Returns (rows, file name, stale): `stale` says that the kernel source the counters were captured on (column
+    `kernels_blob` = git hash-object of csrc/frnn_kernels.cuh at capture time) is not the one in the tree now."""
+    for name in COUNTER_FILES:
+        out, blobs = {}, set()
+        try:
+            with open(os.path.join(ROOT, "profiles", name)) as f:
+                for row in csv.DictReader(f):
+                    blobs.add(row.get("kernels_blob") or "")
+                    out[(row["workload"], row["kernel"])] = {k: float(v) for k, v in row.items()
+                                                             if k not in ("workload", "kernel", "profile", "kernels_blob")}
+        except Exception:
+            continue
+        if out:
+            return out, "profiles/" + name, blobs != {blob_hash(KERNELS_SOURCE)}
+    return {}, None, True
+
+
+def _round(v, digits=8):
+    """Floats to `digits` significant digits (the compact line is for reading and parsing, the full report keeps everything)."""
+    if isinstance(v, float):
+        return float(f"{v:.{digits}g}")
+    if isinstance(v, dict):
+        return {k: _round(x, digits) for k, x in v.items()}
+    if isinstance(v, (list, tuple)):
+        return [_round(x, digits) for x in v]
+    return v
+
+
+def _pick(d, keys):
+    return {k: d[k] for k in keys if isinstance(d, dict) and k in d}
+
+
+def _short(text, limit=160):
+    return text if not isinstance(text, str) or len(text) <= limit else text[: limit - 3] + "..."
+
+
+def compact_line(full: dict) -> dict:
+    """The ONE stdout line: the keys of the bench contract and nothing else (the round-2 line carried every leg, grew to
+    21.6 KB and the driver could not read it).  Everything else stays in the full report (FULL_REPORT, stderr)."""
+    line = _pick(full, ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                        "vs_baseline", "dtype", "data", "impl", "gpu_launches", "gpu_launches_per_step", "edges_per_event"))
+    cfg = _pick(full.get("config"), ("workload", "events_per_step", "pool_events_per_gpu", "l2", "grid", "edge_capacity", "parallelism", "sample"))
+    line["config"] = {k: _short(v) for k, v in cfg.items()}
+    if full.get("roofline"):
+        line["roofline"] = _pick(full["roofline"], ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "peak_source", "kernel_us",
+                                                    "dram_frac_of_hbm_peak", "algorithmic_bytes_per_launch", "own_bytes_per_launch",
+                                                    "model_frac_hbm_equivalent", "counters", "counters_stale"))
+        line["roofline"]["peak_source"] = _short(line["roofline"].get("peak_source"), 120)
+    if full.get("cpu_baseline"):
+        line["cpu_baseline"] = _pick(full["cpu_baseline"], ("value", "unit", "cores", "kind", "sample", "ms_per_event"))
+        line["cpu_baseline"]["sample"] = _short(line["cpu_baseline"].get("sample"))
+    if full.get("e2e"):
+        line["e2e"] = _pick(full["e2e"], ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "steps", "copy_floor_ms",
+                                          "e2e_verified", "events_verified"))
+    if full.get("clocks"):
+        line["clocks"] = _pick(full["clocks"], ("sm_mhz", "sm_max_mhz", "reasons", "samples"))
+    if "full_report" in full:
+        line["full_report"] = full["full_report"]
+    return _round(line)
+
+
+def emit(full: dict, out=None, err=None, path: str | None = FULL_REPORT) -> str:
+    """Full report to `path` (if it can be written) and to stderr, then the compact line as the LAST thing on stdout."""
+    out, err = out or sys.stdout, err or sys.stderr
+    full = dict(full)
+    if path:
+        try:
+            os.makedirs(os.path.dirname(os.path.join(ROOT, path)) or ".", exist_ok=True)
+            with open(os.path.join(ROOT, path), "w") as f:
+                json.dump(full, f)
+            full["full_report"] = path
+        except OSError:
+            full["full_report"] = "stderr"
+    else:
+        full["full_report"] = "stderr"
+    print(json.dumps({"full_report": full}), file=err, flush=True)
+    text = json.dumps(compact_line(full))
+    print(text, file=out, flush=True)
+    return text
 
 
 def candidate_rows(x: np.ndarray, r: float, dims: int, bits: int) -> int:
@@ -450,7 +541,7 @@ def main() -> None:
         timeline_us = timeline_of(step, shared, n, 1, args.timeline_steps)
 
     # ---- rooflines of the dominant kernel (the search pass)
-    counters = ncu_counters()
+    counters, counters_file, counters_stale = ncu_counters()
     dims, bits = F.frnn_get_grid(n, 1, 8)
     acct = [0, 1, 2, 3][: len(host_events)]
     cand = float(np.mean([candidate_rows(host_events[i], r, dims, bits) for i in acct]))
@@ -470,7 +561,7 @@ def main() -> None:
                      "l2_bytes_per_launch": c.get("l2_bytes"), "traffic": c.get("dram_bytes"),
                      "dram_gbs": (c["dram_bytes"] / (dur_us * 1e-6) / 1e9) if c.get("dram_bytes") else None,
                      "dram_frac_of_hbm_peak": (c["dram_bytes"] / (dur_us * 1e-6) / 1e9 / peak) if c.get("dram_bytes") else None,
-                     "kernel_us": dur_us, "counters": "profiles/r02_counters.csv (ncu, one launch, cold cache)",
+                     "kernel_us": dur_us, "counters": f"{counters_file} (ncu, one launch, cold cache)", "counters_stale": counters_stale,
                      "ncu_cold": {"issue_active_pct": c.get("issue_active_pct"), "l1tex_pct_of_peak": c.get("l1tex_pct"), "l2_hit_pct": c.get("l2_hit_pct"),
                                   "occupancy_pct": c.get("occupancy_pct"), "sm_active_over_elapsed": (c["sm_active_cycles"] / c["sm_elapsed_cycles"]) if c.get("sm_elapsed_cycles") else None,
                                   "note": "the L1 data pipe (one wavefront per lane for the survivors' random 32-byte rows) is the busiest unit; neither it nor the "
@@ -483,17 +574,20 @@ def main() -> None:
                      "traffic": c.get("dram_bytes") if c else None,
                      "note": "north_star's definition (bytes of candidate rows of the grid run + hit records over the HBM peak).  The rows are served by "
                              "L2/L1 and ~85 % of the candidates are rejected on a 4-byte key without touching their row, so this is an HBM-EQUIVALENT "
-                             "rate, NOT a fraction of a physical limit (it can exceed 1); the physical bound is roofline / roofline_issue"}
+                             "rate, NOT a fraction of a physical limit (it can exceed 1); the physical bound is `roofline`"}
         return issue, model
 
     dom = "search"
     dom_us = (timeline_us or {}).get(dom, {}).get("dur") or (phases_us or {}).get(dom)
     roofline, roofline_model = rooflines("cfg2", dom, dom_us, cand * 32.0 + 8.0 * e_mean)
     if roofline is None:          # no counters file: still report the model figure as the roofline entry, flagged
-        roofline = dict(roofline_model or {}, note2="profiles/r02_counters.csv missing: issue roofline unavailable")
+        roofline = dict(roofline_model or {}, note2="no profiles/r0N_counters.csv: issue roofline unavailable")
     if roofline is not None and dom_us:
         roofline["kernel_us_source"] = "in-graph %globaltimer timeline" if (timeline_us or {}).get(dom) else "per-phase CUDA events (upper bound)"
         roofline["kernel_us_cuda_events"] = (phases_us or {}).get(dom)
+        if roofline_model and roofline is not roofline_model:      # north_star's byte model beside the physical bound, flagged as what it is
+            roofline["algorithmic_bytes_per_launch"] = roofline_model["algorithmic_bytes_per_launch"]
+            roofline["model_frac_hbm_equivalent"] = roofline_model["frac"]
     path_bytes = cand * 32.0 + 12.0 * e_mean
     path_bytes_g3 = cand_g3 * 32.0 + 12.0 * e_mean
     t_event = ms_local / args.steps * 1e-3          # this rank's seconds per event
@@ -702,13 +796,19 @@ def main() -> None:
             return dt_, got_edges
 
         dt, p_edges = run_pipeline([n] * args.e2e_steps)
-        # one event of the timed loop against the oracle (outside the timed region): the last event submitted
+        # the last depth + 1 events of the timed loop against the oracle (outside the timed region): every host buffer set
+        # still holds the result of the last event that was written into it
         last = args.e2e_steps - 1
-        s_, d_, q_, c_ = hb[last % len(hb)]
-        e_last = int(c_[0])
-        exp = oracle.frnn(host_events[last % n_pin], r, k_max, oracle.CELLS)
-        verified = bool(e_last == exp.count and np.array_equal(s_[:e_last].numpy(), exp.src) and np.array_equal(d_[:e_last].numpy(), exp.dst)
-                        and np.array_equal(q_[:e_last].numpy().view(np.uint32), exp.d2.view(np.uint32)))
+        verified, events_verified = True, 0
+        for ev in range(max(last - len(hb) + 1, 0), last + 1):
+            s_, d_, q_, c_ = hb[ev % len(hb)]
+            e_last = int(c_[0])
+            exp = oracle.frnn(host_events[ev % n_pin], r, k_max, oracle.CELLS)
+            verified = verified and bool(e_last == exp.count and np.array_equal(s_[:e_last].numpy(), exp.src)
+                                         and np.array_equal(d_[:e_last].numpy(), exp.dst)
+                                         and np.array_equal(q_[:e_last].numpy().view(np.uint32), exp.d2.view(np.uint32)))
+            events_verified += 1
+        # (the band report below is that of the last event: s_, d_, q_, e_last and exp are left at it)
         # north_star's acceptance rule: membership may differ only for pairs with |d2 - r2| <= 1e-6 r2, and those must be reported
         r2f = float(np.float32(r) * np.float32(r))
         got_keys = s_[:e_last].numpy().astype(np.int64) << 32 | d_[:e_last].numpy().astype(np.int64)
@@ -746,7 +846,8 @@ def main() -> None:
                "d2h_bytes_per_step": int(8 + 12 * p_edges / args.e2e_steps), "ms_per_step": 1e3 * dt / args.e2e_steps,
                "steps": args.e2e_steps, "api": f"frnn_host_pipeline_submit/wait, depth {depth}: pinned host buffers in and out (src | dst | d2 of an event in one "
                "block: one 2-D copy per event), copies of consecutive events overlap", "timer": "host wall clock around the submit loop + wait",
-               "e2e_verified": verified, "band_report": band_report, "verified_how": "the last event of the timed loop, edges and d2 bit for bit against the oracle (outside the timed region)",
+               "e2e_verified": verified, "events_verified": events_verified, "band_report": band_report,
+               "verified_how": f"the last {events_verified} events of the timed loop (one per host buffer set), edges and d2 bit for bit against the oracle (outside the timed region)",
                "copy_floor_ms": 1e3 * dt_copy / args.e2e_steps,
                "copy_floor_note": f"the same H2D ({n * 32} B) + D2H ({12 * e_avg} B) per event over {depth} streams, pinned buffers, no build: what the "
                                   "box's PCIe link allows",
@@ -787,7 +888,7 @@ def main() -> None:
                              f"{len(seeds) * cap * 12 / 1e6:.0f} MB out > 126 MB L2); no explicit flush",
                        "call_signature": "every step differs from the previous one in its input and output pointers: the graph's node parameters are rewritten every step",
                        "grid": {"dims": dims, "bits": bits}, "edge_capacity": cap, "parallelism": f"events sharded over {rank.world_size} GPU(s), no collective"},
-            "edges_per_event": e_mean, "roofline": roofline, "roofline_issue": roofline if (roofline or {}).get("bound") == "alu" else None,
+            "edges_per_event": e_mean, "roofline": roofline,
             "roofline_model": roofline_model, "path_roofline": path_roofline, "phases_us": phases_us, "timeline_us": timeline_us,
             "varying_n": varying, "k_binding": k_binding, "radius_sweep": radius_sweep,
             "cpu_baseline": cpu_baseline, "e2e": e2e, "next_rows": next_rows, "other_configs": other, "two_streams": two_streams, "gpu_launches": launches_per_step * args.steps,
@@ -795,7 +896,7 @@ def main() -> None:
             "host_wall_ms_per_step": 1e3 * (t1 - t0) / args.steps,
             "paper_context": "paper: 0.04 +- 0.01 s/event on V100 16 GB (PAPER.md:77 Table 1 'FRNN' column), TrackML events; other machine, other data",
         }
-        print(json.dumps(line), flush=True)
+        emit(line)
     D.finalize(rank)
 
 
