@@ -198,6 +198,37 @@ def test_brute_equals_cells_cfg2_sampled_queries():
                 oracle.frnn(x, cfg.r, cfg.k_max, oracle.CELLS, queries=q))
 
 
+@pytest.mark.slow
+def test_brute_equals_cells_cfg3_event0_sampled_queries():
+    """SURVEY.md 8(c) P1/P2 at config 3's size: event 0 of the 16-event batch (the event the batched GPU parity leans on),
+    the definition (section 3.4, quadratic) against the cell list on 4,000 sampled queries."""
+    cfg = events.CONFIGS[3]
+    xb, off = events.make_batch(cfg)
+    x = np.ascontiguousarray(xb[off[0]:off[1]])
+    assert len(x) == cfg.n
+    q = np.sort(np.random.default_rng(3).choice(len(x), 4000, replace=False))
+    a = oracle.frnn(x, cfg.r, cfg.k_max, oracle.BRUTE, queries=q)
+    assert a.count > 4000                                       # mean degree ~2.8: the sample is not empty
+    assert same(a, oracle.frnn(x, cfg.r, cfg.k_max, oracle.CELLS, queries=q))
+
+
+@pytest.mark.slow
+def test_brute_equals_cells_cfg4_sampled_queries():
+    """The same at config 4's parameters (N = 10^6, r = 0.12, sigma = 0.05, K = 512: the dense regime), 2,000 sampled
+    queries = 2 * 10^9 pair evaluations of the definition; and once with a K that binds on most of these rows."""
+    cfg = events.CONFIGS[4]
+    x = events.make_event(cfg)
+    assert len(x) == 1000000
+    q = np.sort(np.random.default_rng(4).choice(cfg.n, 2000, replace=False))
+    a = oracle.frnn(x, cfg.r, cfg.k_max, oracle.BRUTE, queries=q)
+    b = oracle.frnn(x, cfg.r, cfg.k_max, oracle.CELLS, queries=q)
+    assert a.count > 2000 and same(a, b)
+    k = 2
+    assert int((a.uncapped > k).sum()) > 50                      # the cap decides on these rows
+    qk = q[a.uncapped > k]
+    assert same(oracle.frnn(x, cfg.r, k, oracle.BRUTE, queries=qk), oracle.frnn(x, cfg.r, k, oracle.CELLS, queries=qk))
+
+
 def test_low_dimensional_inputs_and_other_dims():
     for dim in (1, 2, 3, 5):
         x = events.uniform_points(500, dim, -1, 1, 3)
