@@ -99,6 +99,7 @@ static void hv_push(hitvec* h, float d2, int32_t j) {
 
 /* Steps 2 and 3 of the definition on the collected S_i.  Returns the kept length. */
 static int64_t cap_and_order(hitvec* h, int k_max) {
+    if (h->len == 0) return 0;                 /* S_i empty: nothing to order (and h->v may still be NULL: not for qsort) */
     if (h->len > k_max) {
         qsort(h->v, (size_t)h->len, sizeof(hit_t), cmp_d2_then_j);
         h->len = k_max;
