@@ -177,15 +177,17 @@ int frnn_label_components(int64_t n, const int32_t* src, const int32_t* dst, con
         if (n_components && cudaMemsetAsync(n_components, 0, 4, st) != cudaSuccess) return FRNN_ERR_CUDA;
         return FRNN_OK;
     }
-    // the three kernels as a plan: on a non-default stream they replay the graph that belongs to the labels array
-    // (node parameters rewritten when the edge list or the threshold changed), else they are launched one by one
+    // the three kernels as a plan: on a non-default stream they replay the graph that belongs to that STREAM (every
+    // argument, the labels array included, is a node parameter rewritten when it changed: a consumer that rotates its
+    // label arrays keeps one graph instead of building one per array and pushing the build graphs out of the cache),
+    // else they are launched one by one
     thread_local frnn::Plan plan;
     plan.clear();
     const CcArgs a{labels, n, src, dst, score, threshold, edge_count, edge_max, n_components};
     plan.add(frnn::fptr(cc_init_kernel), blocks_for(n, 256, 0x7fffffff), 1, 256, 0, a);
     if (edge_max > 0) plan.add(frnn::fptr(cc_hook_kernel), blocks_for(edge_max, 256, 148 * 64), 1, 256, 0, a);
     plan.add(frnn::fptr(cc_flatten_kernel), blocks_for(n, 256, 0x7fffffff), 1, 256, 0, a);
-    return frnn::run_plan(plan, labels, st, frnn::default_use_graph());
+    return frnn::run_plan(plan, cuda_stream, st, frnn::default_use_graph());
 }
 
 }  // extern "C"

@@ -69,6 +69,28 @@ def test_components_long_path_star_and_random(F):
     assert np.array_equal(got, exp) and nc == nc_exp
 
 
+def test_components_rotating_label_arrays_replay_one_graph(F):
+    """A consumer that writes every event's labels into a different array (here 80 of them, more than the 64 graph
+    executables the library keeps) must not pay a graph build per call: the graph belongs to the stream and the
+    labels pointer is one more node parameter.  Results are checked for every array."""
+    n = 5000
+    graphs = [events.random_graph(n, 3000 + 10 * k, 100 + k) for k in range(4)]
+    exps = [NO.label_components(n, s, d) for s, d in graphs]
+    dg = [(dev(s), dev(d)) for s, d in graphs]
+    st = torch.cuda.Stream()
+    labels = [torch.empty(n, dtype=torch.int32, device="cuda") for _ in range(80)]
+    ncs = torch.zeros(80, dtype=torch.int32, device="cuda")
+    torch.cuda.synchronize()
+    F.frnn_label_components(n, *dg[0], labels=labels[0], n_components=ncs[0:1], stream=st)     # first call on this stream: may build
+    b0 = F.frnn_graph_builds()
+    for k in range(80):
+        F.frnn_label_components(n, *dg[k % 4], labels=labels[k], n_components=ncs[k:k + 1], stream=st)
+    st.synchronize()
+    assert F.frnn_graph_builds() == b0
+    for k in range(80):
+        assert np.array_equal(labels[k].cpu().numpy(), exps[k % 4][0]) and int(ncs[k].item()) == exps[k % 4][1], k
+
+
 def test_components_degenerate_and_device_count(F):
     got, nc = gpu_labels(F, 7, np.zeros(0, np.int32), np.zeros(0, np.int32))
     assert np.array_equal(got, np.arange(7)) and nc == 7
