@@ -86,13 +86,20 @@ const char* frnn_last_error_string(void);
  *               cuda_stream and SYNCHRONISES that stream once (about 60 us), then enqueues the build on the grid it picked;
  *               grid_bits is ignored; the workspace must hold frnn_workspace_bytes_opt() with the same options (room for any
  *               grid the call may pick).  For streams whose statistics really change from event to event; otherwise choose
- *               once with frnn_suggest_grid and reuse the options.
+ *               once with frnn_suggest_grid and reuse the options.  A stream that is being captured cannot be
+ *               synchronised: the call then returns FRNN_ERR_UNSUPPORTED (so do frnn_suggest_grid / _bin_order).
  *   grid_bits   log2 of the toroidal grid extent per binned coordinate, 2..8; 0 = automatic (5).  With fewer cells
  *               than the data's extent / r, far-apart cells alias onto one table entry: exact, more candidates.
  *   order       order[0..order_count) = coordinates (0..15, distinct) binned first and keyed next, as in
  *               frnn_set_bin_order; order_count = 0: the first grid_dims coordinates are binned, the next four keyed
  *   launch_mode FRNN_LAUNCH_DEFAULT (process default, see frnn_set_graph_mode), FRNN_LAUNCH_GRAPH, FRNN_LAUNCH_PLAIN
- *   timeline    != 0: the kernels leave %globaltimer stamps in the workspace (frnn_get_timeline)
+ *   timeline    != 0: the kernels leave %globaltimer stamps in the workspace (frnn_get_timeline); 0 leaves the
+ *               process-wide setting (frnn_set_profiling(2)) as it is
+ * What a non-NULL options argument inherits from the process-wide setters: launch_mode 0 takes frnn_set_graph_mode's
+ * default and timeline 0 takes frnn_set_profiling(2)'s; the GRID and the coordinate ORDER are never inherited -- grid_dims
+ * 0 / grid_bits 0 / order_count 0 mean "from the event size" / 5 / "the default order" even after frnn_set_grid or
+ * frnn_set_bin_order (those two only serve calls made without options).  frnn_get_grid_opt reports the grid a call
+ * with given options runs on.
  * struct_bytes must be sizeof(frnn_options) of the caller's header (frnn_options_init sets it).
  */
 enum { FRNN_LAUNCH_DEFAULT = 0, FRNN_LAUNCH_GRAPH = 1, FRNN_LAUNCH_PLAIN = 2 };
@@ -128,6 +135,9 @@ size_t frnn_workspace_bytes_opt(const frnn_options* opt, int64_t n_total, int n_
 int frnn_set_grid(int grid_dims, int grid_bits);
 /* The grid a call without options over (n_total, n_events, dim) would use. */
 void frnn_get_grid(int64_t n_total, int n_events, int dim, int* grid_dims, int* grid_bits);
+/* The same for a call made with `opt` (NULL: frnn_get_grid).  FRNN_GRID_AUTO or invalid options: both outputs are set to 0
+ * (the grid is then only known per call). */
+void frnn_get_grid_opt(const frnn_options* opt, int64_t n_total, int n_events, int dim, int* grid_dims, int* grid_bits);
 
 /*
  * S1 from the data (section 3.4: the O(3^k k n) trade-off behind the paper's
@@ -362,8 +372,9 @@ const char* frnn_phase_name(int phase);
  * In-graph timeline.  frnn_set_profiling(2) (instead of 1) keeps the CUDA-graph replay and makes every
  * kernel of later calls leave the earliest start and the latest end of its warps (%globaltimer) in the
  * call's workspace; frnn_get_timeline synchronises nothing itself (the caller waits for the call first),
- * copies the stamps of the LAST call that used `workspace` (a device pointer; n_total / n_events / dim as in
- * that call) and writes, per kernel (bin, scan_cells, scatter, search, emit), begin and end in
+ * copies the stamps of the LAST call that used `workspace` (a device pointer: the base the call was given.  The stamps
+ * sit at a fixed offset from it, so the call may have been made with any options -- per-call grid, coordinate order,
+ * FRNN_GRID_AUTO; n_total / n_events / dim are only checked for plausibility) and writes, per kernel (bin, scan_cells, scatter, search, emit), begin and end in
  * microseconds relative to the start of the first kernel.  Returns the number of kernels written or a
  * negative status.  Unlike mode 1 this does not perturb the launch sequence.
  */
@@ -399,6 +410,9 @@ int frnn_gather_edge_rows(const float* points, int64_t n, int dim, const int32_t
  * All pointers are DEVICE pointers (labels int32[n], n_components int32[1], edge_count int64[1] or NULL).
  * Edges with an end point outside [0, n) and self loops are ignored.  No workspace: labels doubles as the
  * union-find parent array.  Asynchronous on cuda_stream.  Returns FRNN_OK or a negative status.
+ * On a non-default stream the three kernels replay one CUDA graph that belongs to the STREAM; labels, the edge arrays
+ * and every other argument are rewritten in its nodes when they change (frnn_graph_builds does not move when a
+ * consumer rotates its arrays).  Calls that share a stream must come from one host thread at a time.
  */
 int frnn_label_components(int64_t n, const int32_t* src, const int32_t* dst, const float* score, float threshold,
                           const int64_t* edge_count, int64_t edge_max, int32_t* labels, int32_t* n_components,

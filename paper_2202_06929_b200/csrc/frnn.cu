@@ -32,6 +32,8 @@ constexpr float kCellSlack = 1.0078125f;   // 1 + 2^-7, see cell_coord()
 constexpr size_t kAlign = 256;
 constexpr int64_t kPrefixTilesMin = 1024;   // above this many emit tiles the tile offsets come from tile_prefix_kernel
 constexpr int kTimelinePhases = 5;
+constexpr size_t kCountersBytes = 256;      // head of every workspace (see make_layout)
+constexpr size_t kStampsOffset = 64;        // of the timeline stamps inside it
 const char* const kTimelineNames[kTimelinePhases] = {"bin", "scan_cells", "scatter", "search", "emit"};
 constexpr int kPhases = 6;
 const char* const kPhaseNames[kPhases] = {"memset", "bin", "scan_cells", "scatter", "search", "emit"};
@@ -96,7 +98,7 @@ int opts_from(const frnn_options* in, Opts* out) {
         if (rc != FRNN_OK) return rc;
         if (in->launch_mode == FRNN_LAUNCH_GRAPH) o.use_graph = true;
         if (in->launch_mode == FRNN_LAUNCH_PLAIN) o.use_graph = false;
-        o.timeline = in->timeline != 0;
+        if (in->timeline != 0) o.timeline = true;            // 0 keeps the process-wide setting (frnn_set_profiling(2))
     }
     *out = o;
     return FRNN_OK;
@@ -153,9 +155,11 @@ Layout make_layout(int64_t n_total, int n_events, GridChoice g, int dim, bool or
     L.scan_blocks = (n_rows + L.rows_per_block - 1) / L.rows_per_block;
     L.emit_tiles = (n_total + kEmitThreads - 1) / kEmitThreads;
     size_t o = 0;
+    // the counters block is the HEAD of the workspace: its offset depends on nothing (not on the grid, the options or n), so
+    // frnn_get_timeline finds the stamps of a call whatever options that call was made with (FRNN_GRID_AUTO included)
+    L.off_counters = o; o = align_up(o + kCountersBytes);   // [0..3] cursor of the cell scan (u32); [64..) timeline stamps (u64 x 2 x kTimelinePhases)
     L.off_cells = o;    o = align_up(o + static_cast<size_t>(L.n_entries + 8) * 4);
     L.off_tiles = o;    o = align_up(o + static_cast<size_t>(L.emit_tiles > 0 ? L.emit_tiles : 1) * 8 * kDegSlices);
-    L.off_counters = o; o = align_up(o + 256);         // [0..3] cursor of the cell scan (u32); [64..) timeline stamps (u64 x 2 x kTimelinePhases)
     const size_t n = static_cast<size_t>(n_total > 0 ? n_total : 1);
     L.off_cnt = o;      o = align_up(o + n * 4);       // zeroed: the search pass counts with atomics
     L.zero_bytes = o;
@@ -228,7 +232,7 @@ void make_plan(const Call& c, const Layout& L, Plan& P) {
     uint32_t* cells = reinterpret_cast<uint32_t*>(ws + L.off_cells);
     unsigned long long* tile_deg = reinterpret_cast<unsigned long long*>(ws + L.off_tiles);
     unsigned int* cursor = reinterpret_cast<unsigned int*>(ws + L.off_counters);
-    unsigned long long* stamps = c.opts.timeline ? reinterpret_cast<unsigned long long*>(ws + L.off_counters + 64) : nullptr;
+    unsigned long long* stamps = c.opts.timeline ? reinterpret_cast<unsigned long long*>(ws + L.off_counters + kStampsOffset) : nullptr;
     uint32_t* pcell = reinterpret_cast<uint32_t*>(ws + L.off_pcell);
     uint32_t* prank = reinterpret_cast<uint32_t*>(ws + L.off_prank);
     float4* spts = reinterpret_cast<float4*>(ws + L.off_spts);
@@ -707,24 +711,28 @@ __global__ void __launch_bounds__(1024) suggest_kernel(SuggestArgs k) {
     if (threadIdx.x == 0) k.out->sampled = s_total;
 }
 
-// one page-locked result block per process (the kernel writes it through its device alias), guarded by a mutex
-SuggestOut* g_suggest_host = nullptr;
-std::mutex g_suggest_mutex;
+// One page-locked result block per HOST THREAD (the kernel writes it through its device alias; 17 KB, allocated by the
+// thread's first call and kept): calls from different threads share nothing, so they wait only for their own stream,
+// as include/frnn.h promises for calls on distinct workspaces.
+thread_local SuggestOut* t_suggest_host = nullptr;
 
 int run_suggest(const float* points, int64_t n, int dim, float r, cudaStream_t st, SuggestOut* result) {
-    std::lock_guard<std::mutex> lock(g_suggest_mutex);
-    if (!g_suggest_host) CK(cudaHostAlloc(reinterpret_cast<void**>(&g_suggest_host), sizeof(SuggestOut), cudaHostAllocMapped));
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;       // the estimate synchronises the stream: not while it is being captured
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+    if (cs != cudaStreamCaptureStatusNone) return FRNN_ERR_UNSUPPORTED;
+    if (!t_suggest_host) CK(cudaHostAlloc(reinterpret_cast<void**>(&t_suggest_host), sizeof(SuggestOut), cudaHostAllocMapped));
     SuggestOut* dev = nullptr;
-    CK(cudaHostGetDevicePointer(reinterpret_cast<void**>(&dev), g_suggest_host, 0));
+    CK(cudaHostGetDevicePointer(reinterpret_cast<void**>(&dev), t_suggest_host, 0));
     SuggestArgs a;
     a.pts = points; a.n = n; a.dim = dim;
     a.inv_cell = 1.0f / fmaxf(r * kCellSlack, 1e-30f);
-    a.stride = n > 65536 ? n / 65536 : 1;                          // a sample of at most ~65k points
+    a.stride = (n + 65535) / 65536;                                // every stride-th row: at most 65,536 rows
+    if (a.stride < 1) a.stride = 1;
     a.out = dev;
     suggest_kernel<<<1, 1024, 0, st>>>(a);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(st));
-    *result = *g_suggest_host;
+    *result = *t_suggest_host;
     return FRNN_OK;
 }
 
@@ -803,7 +811,7 @@ int auto_grid(const float* points, int64_t n, int n_events, int dim, float r, cu
 // would read and write the wrong memory.  Host code therefore asks the runtime for the real address, once per
 // device and with that device current (static_scratch_for_current_device), and passes that to the kernels.
 // ------------------------------------------------------------------------------------------------
-constexpr size_t kStaticScratchBytes = 3u << 20;          // 3 MiB: the 8192-row, dim 9..16 layout needs 2,923,520 bytes
+constexpr size_t kStaticScratchBytes = 3u << 20;          // 3 MiB: the 8192-row, dim 9..16 layout needs 2,923,776 bytes
 static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
 
 namespace {
@@ -881,6 +889,15 @@ int frnn_set_grid(int grid_dims, int grid_bits) {
 
 void frnn_get_grid(int64_t n_total, int n_events, int dim, int* grid_dims, int* grid_bits) {
     const GridChoice g = choose_grid(default_opts(), n_total, n_events < 1 ? 1 : n_events, (dim < 1 || dim > kDimMax) ? kDim : dim);
+    if (grid_dims) *grid_dims = g.dims;
+    if (grid_bits) *grid_bits = g.bits;
+}
+
+void frnn_get_grid_opt(const frnn_options* opt, int64_t n_total, int n_events, int dim, int* grid_dims, int* grid_bits) {
+    Opts o;
+    GridChoice g{0, 0};
+    if (opts_from(opt, &o) == FRNN_OK && !o.auto_grid)
+        g = choose_grid(o, n_total, n_events < 1 ? 1 : n_events, (dim < 1 || dim > kDimMax) ? kDim : dim);
     if (grid_dims) *grid_dims = g.dims;
     if (grid_bits) *grid_bits = g.bits;
 }
@@ -1364,10 +1381,9 @@ int frnn_get_profile(float* phase_ms, int max_phases) {
 
 int frnn_get_timeline(const void* workspace, int64_t n_total, int n_events, int dim, double* begin_us, double* end_us, int max_phases) {
     if (!workspace || !begin_us || !end_us || n_total <= 0 || n_events < 1 || dim < 1 || dim > kDimMax) return FRNN_ERR_INVALID_ARG;
-    const Opts o = default_opts();
-    const Layout L = make_layout(n_total, n_events, choose_grid(o, n_total, n_events, dim), dim, o.order.on != 0);
-    unsigned long long h[2 * kTimelinePhases];
-    CK(cudaMemcpy(h, static_cast<const char*>(workspace) + L.off_counters + 64, sizeof(h), cudaMemcpyDeviceToHost));
+    static_assert(kStampsOffset + 2 * kTimelinePhases * 8 <= kCountersBytes, "the stamps fit the counters block");
+    unsigned long long h[2 * kTimelinePhases];              // the stamps sit at a fixed offset from the workspace's base (make_layout)
+    CK(cudaMemcpy(h, static_cast<const char*>(workspace) + kStampsOffset, sizeof(h), cudaMemcpyDeviceToHost));
     const int n = max_phases < kTimelinePhases ? max_phases : kTimelinePhases;
     const unsigned long long t0 = ~h[0];                   // start of the first kernel
     for (int i = 0; i < n; ++i) {

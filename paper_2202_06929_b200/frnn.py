@@ -66,6 +66,7 @@ _SIGNATURES = {
     "frnn_workspace_bytes_opt": (_c.c_size_t, [_OPT, _c.c_int64, _c.c_int, _c.c_int, _c.c_int]),
     "frnn_set_grid": (_c.c_int, [_c.c_int, _c.c_int]),
     "frnn_get_grid": (None, [_c.c_int64, _c.c_int, _c.c_int, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int)]),
+    "frnn_get_grid_opt": (None, [_OPT, _c.c_int64, _c.c_int, _c.c_int, _c.POINTER(_c.c_int), _c.POINTER(_c.c_int)]),
     "frnn_suggest_grid": (_c.c_int, [_c.c_void_p, _c.c_int64, _c.c_int, _c.c_int, _c.c_float, _c.c_int, _OPT, _c.POINTER(FrnnGridReport),
                                      _c.c_void_p]),
     "frnn_build_opt": (_c.c_int, [_OPT] + _BUILD_ARGS),
@@ -180,6 +181,13 @@ def frnn_set_grid(grid_dims: int = 0, grid_bits: int = 0) -> None:
 def frnn_get_grid(n_total: int, n_events: int = 1, dim: int = 8) -> tuple[int, int]:
     d, b = _c.c_int(0), _c.c_int(0)
     lib().frnn_get_grid(int(n_total), int(n_events), int(dim), _c.byref(d), _c.byref(b))
+    return d.value, b.value
+
+
+def frnn_get_grid_opt(opt: FrnnOptions | None, n_total: int, n_events: int = 1, dim: int = 8) -> tuple[int, int]:
+    """(grid_dims, grid_bits) a call made with ``opt`` runs on; (0, 0) for FRNN_GRID_AUTO (chosen per call)."""
+    d, b = _c.c_int(0), _c.c_int(0)
+    lib().frnn_get_grid_opt(_opt_ref(opt), int(n_total), int(n_events), int(dim), _c.byref(d), _c.byref(b))
     return d.value, b.value
 
 

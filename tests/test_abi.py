@@ -55,6 +55,16 @@ def test_host_only_entry_points():
         frnn.frnn_set_grid(0, 0)
     d, b = frnn.frnn_get_grid(120000)
     assert 1 <= d <= 6 and 2 <= b <= 8
+    # options never inherit frnn_set_grid's default; frnn_get_grid_opt says what a call with options runs on
+    try:
+        frnn.frnn_set_grid(2, 7)
+        assert frnn.frnn_get_grid(120000) == (2, 7)
+        assert frnn.frnn_get_grid_opt(frnn.frnn_options(), 120000) == (d, b)
+        assert frnn.frnn_get_grid_opt(frnn.frnn_options(3, 6), 120000) == (3, 6)
+        assert frnn.frnn_get_grid_opt(None, 120000) == (2, 7)
+        assert frnn.frnn_get_grid_opt(frnn.frnn_options(frnn.FRNN_GRID_AUTO), 120000) == (0, 0)
+    finally:
+        frnn.frnn_set_grid(0, 0)
     assert frnn.frnn_get_grid(120000, 1, 2)[0] == 2                    # never more binned coordinates than the rows have
     # the linear cell id (event, cell) must fit 32 bits for any batch size
     d, b = frnn.frnn_get_grid(120000 * 4096, 4096)

@@ -294,6 +294,32 @@ def test_timeline_mode_gives_the_same_result_and_ordered_stamps(F):
     assert tl["emit"][1] < 1e5                                            # microseconds, not garbage
 
 
+@pytest.mark.parametrize("how", ["grid_3x6", "grid_2x8_order", "auto"])
+def test_timeline_of_calls_made_with_options(F, how):
+    """The stamps sit at the head of the workspace, so frnn_get_timeline reads them whatever grid, coordinate order or
+    launch options the call was made with (it used to derive their offset from the process defaults)."""
+    cfg = events.CONFIGS[1]
+    x = events.make_event(cfg)
+    exp = oracle.frnn(x, cfg.r, cfg.k_max, oracle.CELLS)
+    pts = torch.from_numpy(x).cuda()
+    opt = {"grid_3x6": F.frnn_options(3, 6, timeline=True), "grid_2x8_order": F.frnn_options(2, 8, order=[5, 2, 7], timeline=True),
+           "auto": F.frnn_options(F.FRNN_GRID_AUTO, timeline=True)}[how]
+    assert F.frnn_workspace_bytes(cfg.n, 1, 8, cfg.k_max, opt) != F.frnn_workspace_bytes(cfg.n, 1, 8, cfg.k_max)
+    ws = F.Workspace(cfg.n, 1, cfg.k_max, cfg.n * 8, opt=opt)
+    st = torch.cuda.Stream()
+    res = F.frnn_build_ex(pts, cfg.r, cfg.k_max, ws=ws, stream=st, opt=opt)
+    st.synchronize()
+    tl = F.frnn_get_timeline(ws.buf, cfg.n, 1)
+    s, d, q = (t.cpu().numpy() for t in res.trimmed())
+    assert_same(Got(s, d, q), exp, cfg.r, "timeline with options: " + how)
+    names = list(tl)
+    assert names == ["bin", "scan_cells", "scatter", "search", "emit"]
+    assert tl["bin"][0] == 0.0
+    for a, b in zip(names, names[1:]):
+        assert tl[a][0] < tl[a][1] <= tl[b][0] + 1e-9, (a, b, tl)
+    assert 1.0 < tl["emit"][1] < 1e5                                      # microseconds of a real call, not garbage
+
+
 def test_host_pipeline_overlapped_events(F):
     """frnn_host_pipeline_*: seven events through three slots, results in pinned host buffers, count on the host."""
     cfg = events.CONFIGS[0]
