@@ -317,6 +317,7 @@ def main() -> None:
     ap.add_argument("--other-reps", type=int, default=50, help="repetitions for the other configs / N sweep / K and radius legs")
     ap.add_argument("--next-steps", type=int, default=300, help="timed repetitions of the two edge-list consumers")
     ap.add_argument("--other-configs", default="0,1,3,4,sweep", help="which parts of the `other` leg run (for ncu captures of one config)")
+    ap.add_argument("--k-cases", default="config2,cluster,dense", help="which cases of the k_binding leg run (for ncu captures of one case)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -613,16 +614,18 @@ def main() -> None:
         reps = 4 * args.other_reps
         x2 = host_events[0]
         rows = {}
-        for kk in (256, 16, 4, 2):
+        k_cases = set(args.k_cases.split(","))
+        for kk in (256, 16, 4, 2) if "config2" in k_cases else ():
             ms_, e_, _, _ = time_single(x2, r, kk, reps)
             rows[f"config2_K{kk}"] = {"k_max": kk, "ms_per_event": ms_, "edges": e_}
-        for kk in (256, 4):
+        for kk in (256, 4) if "config2" in k_cases else ():
             rows[f"config2_K{kk}"]["vs_K256"] = rows[f"config2_K{kk}"]["ms_per_event"] / rows["config2_K256"]["ms_per_event"]
-        xc = events.one_cluster(2000, 0.01, 3)
-        ms_, e_, _, _ = time_single(xc, 0.1, 64, reps, cap_rows=64)
-        rows["one_cluster_n2000_K64"] = {"k_max": 64, "ms_per_event": ms_, "edges": e_, "note": "every row has 1999 neighbours: the bisection fallback (count > 512)"}
-        xd = events.dense_tracks(n, 200.0, 0.02, 5)
-        for kk in (64, 512):
+        if "cluster" in k_cases:
+            xc = events.one_cluster(2000, 0.01, 3)
+            ms_, e_, _, _ = time_single(xc, 0.1, 64, reps, cap_rows=64)
+            rows["one_cluster_n2000_K64"] = {"k_max": 64, "ms_per_event": ms_, "edges": e_, "note": "every row has 1999 neighbours: the bisection fallback (count > 512)"}
+        xd = events.dense_tracks(n, 200.0, 0.02, 5) if "dense" in k_cases else None
+        for kk in (64, 512) if "dense" in k_cases else ():
             ms_, e_, _, _ = time_single(xd, 0.1, kk, max(reps // 8, 3), cap_rows=min(kk, 256))
             rows[f"dense_event_n120k_K{kk}"] = {"k_max": kk, "ms_per_event": ms_, "edges": e_, "edges_per_s": e_ / (ms_ * 1e-3),
                                                 "note": "120k points in tracks of Poisson(200) hits, sigma 0.02: mean degree ~170; "

@@ -1082,8 +1082,11 @@ __device__ __forceinline__ unsigned long long warp_select_keys(unsigned long lon
     uint32_t prefix = 0, fixed = 0, kk = k, c_eq = 0;
 #pragma unroll 1
     for (int shift = 24; shift >= 0; shift -= 8) {
-#pragma unroll
-        for (int b = 0; b < 8; ++b) hist[lane * 8 + b] = 0u;
+        // (128-bit accesses: zeroing and reading the lane's 8 bins word by word put the 32 lanes on 4 banks -- an 8-way
+        // conflict on each of 16 instructions per pass, which was most of the kernel's shared-memory wavefronts)
+        uint4* hist4 = reinterpret_cast<uint4*>(hist);
+        hist4[lane] = make_uint4(0u, 0u, 0u, 0u);
+        hist4[lane + 32] = make_uint4(0u, 0u, 0u, 0u);
         __syncwarp();
         for (uint32_t t = lane; t < n; t += 32) {
             const uint32_t d = w[2 * t + 1];
@@ -1091,8 +1094,13 @@ __device__ __forceinline__ unsigned long long warp_select_keys(unsigned long lon
         }
         __syncwarp();
         uint32_t loc[8], sum = 0;
+        {
+            const uint4 lo4 = hist4[2 * lane], hi4 = hist4[2 * lane + 1];
+            loc[0] = lo4.x; loc[1] = lo4.y; loc[2] = lo4.z; loc[3] = lo4.w;
+            loc[4] = hi4.x; loc[5] = hi4.y; loc[6] = hi4.z; loc[7] = hi4.w;
+        }
 #pragma unroll
-        for (int b = 0; b < 8; ++b) { loc[b] = hist[lane * 8 + b]; sum += loc[b]; }
+        for (int b = 0; b < 8; ++b) sum += loc[b];
         uint32_t incl = sum;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -1367,7 +1375,7 @@ __global__ void __launch_bounds__(kEmitThreads, 1024 / kEmitThreads) emit_kernel
     __shared__ uint32_t s_kept[kEmitThreads];              // medium rows: bit h set = stored hit h is among the K nearest
     __shared__ uint32_t s_mwarp[kEmitThreads / 32];
     __shared__ unsigned long long s_stage[kEmitThreads / 32][kStage];   // big rows: per-warp staging of (d2, j) keys
-    __shared__ uint32_t s_hist[kEmitThreads / 32][256];                 // big rows: per-warp histogram of the radix select
+    __shared__ __align__(16) uint32_t s_hist[kEmitThreads / 32][256];                 // big rows: per-warp histogram of the radix select
     __shared__ unsigned int s_done;                        // timeline only: threads of the block that have finished
     if (threadIdx.x == 0) s_done = 0u;                     // (made visible by the barriers below)
     stamp_begin(a.stamps, 4);
