@@ -847,7 +847,7 @@ int static_scratch_for_current_device(void** out) {
 
 extern "C" {
 
-int frnn_version(void) { return 400; }   // 0.4.0
+int frnn_version(void) { return 500; }   // 0.5.0: frnn_build_static, frnn_static_scratch_bytes, frnn_get_grid_opt; counters block at the workspace head
 
 const char* frnn_status_string(int status) {
     switch (status) {
