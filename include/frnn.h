@@ -71,7 +71,8 @@ int frnn_version(void);
 const char* frnn_status_string(int status);
 
 /* Text of the last CUDA failure behind a FRNN_ERR_CUDA returned on THIS host thread ("call: message (name)"; "" if
- * none yet).  The library clears the runtime's non-sticky error state before returning FRNN_ERR_CUDA. */
+ * none yet).  The library clears the runtime's non-sticky error state before returning FRNN_ERR_CUDA.  frnn_build_static
+ * leaves its own sentence here when it refuses an event beyond its size limit (FRNN_ERR_UNSUPPORTED). */
 const char* frnn_last_error_string(void);
 
 /*
